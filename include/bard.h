@@ -1,0 +1,126 @@
+/*
+ * bard.h -- C ABI of the B200-native batched rigid-body operator library (libbard.so).
+ *
+ * Hot path of "Batched Differentiable Rigid Body Dynamics in PyTorch for GPU-Accelerated Robot
+ * Learning" (arxiv 2605.31481, /root/reference/PAPER.md): forward kinematics, geometric Jacobians,
+ * RNEA inverse dynamics and the CRBA mass matrix (operator list PAPER.md:37) for B independent
+ * robot states per call.  The model is immutable and built once; every operator is
+ * one asynchronous kernel launch on the caller's stream.
+ *
+ * Conventions (readings of the paper are listed in DESIGN.md "Readings"):
+ *   - bodies i = 0..nb-1, one joint per body, parent[i] in {-1, 0..i-1}; -1 = world.
+ *   - T_pc,i = T_pre,i * T_J(q_i) * T_post,i maps child to parent coordinates (eq. (1)).
+ *   - joint types: revolute (nq=nv=1), prismatic (1,1), fixed (0,0), free (nq=7, nv=6).
+ *     free joint: q = [p(3), quat x,y,z,w] (normalised inside the kernels), qd = body-frame twist
+ *     [v_lin(3); omega(3)], qdd its component-wise derivative, tau = [force(3); moment(3)].
+ *   - spatial order at the boundary is [linear; angular] (row order of eq. (7)).
+ *   - DEVICE I/O LAYOUT: structure of arrays, batch fastest: component c of env b is ptr[c*B + b].
+ *       q[nq][B]  qd[nv][B]  qdd[nv][B]           inputs,  fp32, device memory
+ *       pose[nb][12][B]   c = 0..8 R row-major (body->world), 9..11 p (world)
+ *       J[nframes][6][nv][B]  rows 0-2 linear, 3-5 angular; geometric Jacobian at the frame origin,
+ *                             world axes (eq. (7) shifted to the frame origin)
+ *       tau[nv][B]        M[nv][nv][B]  (full symmetric matrix, every element written once)
+ *
+ * Ownership: the caller owns every q/qd/qdd/output DEVICE buffer.  The library owns only the model
+ * (host struct + one device constant blob), freed by bard_model_destroy.  Host arrays in
+ * bard_model_desc are copied by bard_model_create.
+ *
+ * Execution: operator calls enqueue exactly one kernel on `stream`, allocate nothing and never
+ * synchronise.  B == 0 returns BARD_OK without a launch.  Outputs are fully overwritten.
+ *
+ * Errors: return codes only; bard_last_error() gives thread-local detail text.
+ */
+#ifndef BARD_H
+#define BARD_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct bard_model bard_model;     /* opaque */
+typedef void* bard_stream;                /* a cudaStream_t (NULL = default stream) */
+
+typedef enum {
+  BARD_OK = 0,
+  BARD_ERR_INVALID_ARG = 1,   /* NULL pointer, negative B, nb < 1, bad joint type, zero axis, mass <= 0,
+                                 non-identity T_post on a free joint, bad frame body */
+  BARD_ERR_TOPOLOGY = 2,      /* parent[i] >= i or < -1 (topological numbering is required) */
+  BARD_ERR_UNSUPPORTED = 3,   /* nb > BARD_MAX_BODIES or nv > BARD_MAX_DOF or B too large */
+  BARD_ERR_ALLOC = 4,
+  BARD_ERR_CUDA = 5           /* failed cudaMalloc/cudaMemcpy/launch; text in bard_last_error() */
+} bard_status;
+
+typedef enum {
+  BARD_JOINT_REVOLUTE = 0, BARD_JOINT_PRISMATIC = 1, BARD_JOINT_FIXED = 2, BARD_JOINT_FREE = 3
+} bard_joint_type;
+
+#define BARD_MAX_BODIES 64
+#define BARD_MAX_DOF    64
+#define BARD_MAX_FRAMES 16
+
+/* Robot description (all HOST pointers, fp64; copied by bard_model_create). */
+typedef struct {
+  int32_t        nb;
+  const int32_t* parent;      /* [nb]   -1 = world; parent[i] < i                                  */
+  const int32_t* joint_type;  /* [nb]   bard_joint_type                                            */
+  const double*  axis;        /* [nb*3] joint frame; normalised by the builder;
+                                 ignored for FIXED / FREE                                          */
+  const double*  T_pre;       /* [nb*12] rows [R|t]: the paper's T_joint (parent body -> joint)    */
+  const double*  T_post;      /* [nb*12] or NULL = identity: the paper's T_link; identity for FREE */
+  const double*  mass;        /* [nb]   > 0                                                        */
+  const double*  com;         /* [nb*3] body frame                                                 */
+  const double*  inertia;     /* [nb*6] xx,xy,xz,yy,yz,zz about the COM, body axes                 */
+  double         gravity[3];  /* world frame, e.g. (0,0,-9.81)                                     */
+} bard_model_desc;
+
+/* Tables exported for bit-exact checks of the level schedule and index tables. */
+enum {
+  BARD_TAB_LEVEL_PTR = 0,   /* int32 [nlevels+1]                                              */
+  BARD_TAB_LEVEL_BODY = 1,  /* int32 [nb]  bodies sorted by (level, body index)                */
+  BARD_TAB_BODY_LEVEL = 2,  /* int32 [nb]                                                     */
+  BARD_TAB_PARENT_SLOT = 3, /* int32 [nb]  slot in LEVEL_BODY of the parent of LEVEL_BODY[s]  */
+  BARD_TAB_Q_OFF = 4,       /* int32 [nb+1]                                                   */
+  BARD_TAB_V_OFF = 5,       /* int32 [nb+1]                                                   */
+  BARD_TAB_DOF_BODY = 6,    /* int32 [nv]                                                     */
+  BARD_TAB_ANC_MASK = 7,    /* uint64 [nb] bit j set <=> j == i or j is an ancestor of i      */
+  BARD_TAB_RODRIGUES = 8    /* float [nb*36] R0 A B (3x3 row-major) t0 a b, eq. (2)-(3)       */
+};
+
+/* Build the immutable model on `cuda_device`: validation, q/v offsets, level schedule, ancestor sets,
+ * Rodrigues constants (eq. (2)-(3); fp64 on the host, rounded once to fp32), motion
+ * subspaces, compact spatial inertias; one upload of the constant blob.  *out is set on BARD_OK only.
+ * cuda_device < 0 builds a HOST-ONLY model (no CUDA call): tables and dims can be queried, every
+ * operator call on it returns BARD_ERR_INVALID_ARG. */
+bard_status bard_model_create(const bard_model_desc* desc, int cuda_device, bard_model** out);
+void        bard_model_destroy(bard_model* m);
+bard_status bard_model_dims(const bard_model* m, int32_t* nb, int32_t* nq, int32_t* nv, int32_t* nlevels);
+/* Copy table `table_id` to host_dst (cap bytes).  *need receives the size in bytes; if cap < need
+ * nothing is copied and BARD_ERR_INVALID_ARG is returned (call with cap 0 to query). */
+bard_status bard_model_get_table(const bard_model* m, int table_id, void* host_dst, size_t cap, size_t* need);
+/* Choose the Jacobian frames: frame f is rigidly attached to body[f] at `offset` (body coordinates,
+ * [nframes*3], NULL = zeros).  Not thread-safe against concurrent bard_jacobian calls. */
+bard_status bard_model_set_frames(bard_model* m, int32_t nframes, const int32_t* body, const double* offset);
+
+/* FK (eq. (1)-(5), level-ordered outward propagation). */
+bard_status bard_fk(const bard_model* m, int64_t B, const float* q, float* pose, bard_stream stream);
+/* Geometric Jacobian of the frames chosen by bard_model_set_frames (eq. (7)). */
+bard_status bard_jacobian(const bard_model* m, int64_t B, const float* q, float* J, bard_stream stream);
+/* RNEA: outward velocity/acceleration pass (eq. (6)) and inward force pass
+ * fused in one launch; gravity enters as a_world = -g. */
+bard_status bard_rnea(const bard_model* m, int64_t B, const float* q, const float* qd, const float* qdd,
+                      float* tau, bard_stream stream);
+/* CRBA: composite-inertia backward sweep (the X^T M X update of PAPER.md:103) and mass-matrix fill. */
+bard_status bard_crba(const bard_model* m, int64_t B, const float* q, float* M, bard_stream stream);
+
+const char* bard_status_string(bard_status s);
+const char* bard_last_error(void);
+/* Number of kernel launches this process has enqueued through the library (bench.py's gpu_launches). */
+int64_t     bard_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

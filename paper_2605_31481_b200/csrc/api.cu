@@ -1,0 +1,143 @@
+// C ABI (include/bard.h): argument checks, table export, dispatch to the kernel launchers.
+#include <cuda_runtime.h>
+
+#include <atomic>
+#include <cstring>
+#include <new>
+
+#include "bard_internal.h"
+
+struct bard_model {
+  bard::Model m;
+};
+
+namespace bard {
+static thread_local std::string g_err;
+std::atomic<int64_t> g_launches{0};
+void set_error(const std::string& s) { g_err = s; }
+bard_status build_model(const bard_model_desc* d, int device, Model& M);
+bard_status set_frames(Model& M, int32_t nframes, const int32_t* body, const double* offset);
+}  // namespace bard
+
+using bard::set_error;
+
+extern "C" {
+
+bard_status bard_model_create(const bard_model_desc* desc, int cuda_device, bard_model** out) {
+  if (!out) { set_error("bard_model_create: out is NULL"); return BARD_ERR_INVALID_ARG; }
+  bard_model* bm = new (std::nothrow) bard_model();
+  if (!bm) { set_error("bard_model_create: host allocation failed"); return BARD_ERR_ALLOC; }
+  bard_status s = bard::build_model(desc, cuda_device, bm->m);
+  if (s != BARD_OK) { delete bm; return s; }
+  *out = bm;
+  return BARD_OK;
+}
+
+void bard_model_destroy(bard_model* bm) {
+  if (!bm) return;
+  if (bm->m.d_blob) {
+    int prev = 0;
+    cudaGetDevice(&prev);
+    cudaSetDevice(bm->m.device);
+    cudaFree(bm->m.d_blob);
+    cudaSetDevice(prev);
+  }
+  delete bm;
+}
+
+bard_status bard_model_dims(const bard_model* bm, int32_t* nb, int32_t* nq, int32_t* nv, int32_t* nlevels) {
+  if (!bm) { set_error("bard_model_dims: model is NULL"); return BARD_ERR_INVALID_ARG; }
+  if (nb) *nb = bm->m.nb;
+  if (nq) *nq = bm->m.nq;
+  if (nv) *nv = bm->m.nv;
+  if (nlevels) *nlevels = bm->m.nlevels;
+  return BARD_OK;
+}
+
+bard_status bard_model_get_table(const bard_model* bm, int table_id, void* host_dst, size_t cap, size_t* need) {
+  if (!bm) { set_error("bard_model_get_table: model is NULL"); return BARD_ERR_INVALID_ARG; }
+  const bard::Model& m = bm->m;
+  const void* src = nullptr;
+  size_t bytes = 0;
+  auto vec32 = [&](const std::vector<int32_t>& v) { src = v.data(); bytes = v.size() * sizeof(int32_t); };
+  switch (table_id) {
+    case BARD_TAB_LEVEL_PTR: vec32(m.level_ptr); break;
+    case BARD_TAB_LEVEL_BODY: vec32(m.level_body); break;
+    case BARD_TAB_BODY_LEVEL: vec32(m.body_level); break;
+    case BARD_TAB_PARENT_SLOT: vec32(m.parent_slot); break;
+    case BARD_TAB_Q_OFF: vec32(m.q_off); break;
+    case BARD_TAB_V_OFF: vec32(m.v_off); break;
+    case BARD_TAB_DOF_BODY: vec32(m.dof_body); break;
+    case BARD_TAB_ANC_MASK: src = m.anc_mask.data(); bytes = m.anc_mask.size() * sizeof(uint64_t); break;
+    case BARD_TAB_RODRIGUES: src = m.rodrigues.data(); bytes = m.rodrigues.size() * sizeof(float); break;
+    default: set_error("bard_model_get_table: unknown table id"); return BARD_ERR_INVALID_ARG;
+  }
+  if (need) *need = bytes;
+  if (cap < bytes || (!host_dst && bytes)) {
+    set_error("bard_model_get_table: destination too small");
+    return BARD_ERR_INVALID_ARG;
+  }
+  if (bytes) std::memcpy(host_dst, src, bytes);
+  return BARD_OK;
+}
+
+bard_status bard_model_set_frames(bard_model* bm, int32_t nframes, const int32_t* body, const double* offset) {
+  if (!bm) { set_error("bard_model_set_frames: model is NULL"); return BARD_ERR_INVALID_ARG; }
+  return bard::set_frames(bm->m, nframes, body, offset);
+}
+
+static bard_status check_call(const char* fn, const bard_model* bm, int64_t B, const void* a, const void* b,
+                              const void* c, const void* d) {
+  if (!bm) { set_error(std::string(fn) + ": model is NULL"); return BARD_ERR_INVALID_ARG; }
+  if (!bm->m.d_blob) { set_error(std::string(fn) + ": host-only model (created with cuda_device < 0)"); return BARD_ERR_INVALID_ARG; }
+  if (B < 0) { set_error(std::string(fn) + ": negative batch size"); return BARD_ERR_INVALID_ARG; }
+  if (B > 0 && (!a || !b || !c || !d)) { set_error(std::string(fn) + ": NULL device pointer"); return BARD_ERR_INVALID_ARG; }
+  if (B > ((int64_t)1 << 31) - 1024) { set_error(std::string(fn) + ": B too large"); return BARD_ERR_UNSUPPORTED; }
+  return BARD_OK;
+}
+
+bard_status bard_fk(const bard_model* bm, int64_t B, const float* q, float* pose, bard_stream stream) {
+  bard_status s = check_call("bard_fk", bm, B, bm && bm->m.nq == 0 ? (const void*)pose : q, pose, pose, pose);
+  if (s != BARD_OK || B == 0) return s;
+  return bard::launch_fk(bm->m, B, q, pose, stream);
+}
+
+bard_status bard_jacobian(const bard_model* bm, int64_t B, const float* q, float* J, bard_stream stream) {
+  bard_status s = check_call("bard_jacobian", bm, B, bm && bm->m.nq == 0 ? (const void*)J : q, J, J, J);
+  if (s != BARD_OK || B == 0) return s;
+  if (bm->m.nframes == 0 || bm->m.nv == 0) return BARD_OK;  // empty output
+  return bard::launch_jacobian(bm->m, B, q, J, stream);
+}
+
+bard_status bard_rnea(const bard_model* bm, int64_t B, const float* q, const float* qd, const float* qdd, float* tau,
+                      bard_stream stream) {
+  if (bm && bm->m.nv == 0) return check_call("bard_rnea", bm, B, bm, bm, bm, bm);  // nothing to write
+  bard_status s = check_call("bard_rnea", bm, B, q, qd, qdd, tau);
+  if (s != BARD_OK || B == 0) return s;
+  return bard::launch_rnea(bm->m, B, q, qd, qdd, tau, stream);
+}
+
+bard_status bard_crba(const bard_model* bm, int64_t B, const float* q, float* M, bard_stream stream) {
+  if (bm && bm->m.nv == 0) return check_call("bard_crba", bm, B, bm, bm, bm, bm);
+  bard_status s = check_call("bard_crba", bm, B, q, M, M, M);
+  if (s != BARD_OK || B == 0) return s;
+  return bard::launch_crba(bm->m, B, q, M, stream);
+}
+
+const char* bard_status_string(bard_status s) {
+  switch (s) {
+    case BARD_OK: return "BARD_OK";
+    case BARD_ERR_INVALID_ARG: return "BARD_ERR_INVALID_ARG";
+    case BARD_ERR_TOPOLOGY: return "BARD_ERR_TOPOLOGY";
+    case BARD_ERR_UNSUPPORTED: return "BARD_ERR_UNSUPPORTED";
+    case BARD_ERR_ALLOC: return "BARD_ERR_ALLOC";
+    case BARD_ERR_CUDA: return "BARD_ERR_CUDA";
+  }
+  return "BARD_ERR_UNKNOWN";
+}
+
+const char* bard_last_error(void) { return bard::g_err.c_str(); }
+
+int64_t bard_launch_count(void) { return bard::g_launches.load(); }
+
+}  // extern "C"

@@ -1,0 +1,295 @@
+// Host-side model builder: validation, offsets, level schedule, ancestor masks, Rodrigues
+// constants (eq. (2)-(3)), motion subspaces, compact inertias, slot allocation for the
+// outward sweeps, and the single upload of the constant blob.  All precompute is fp64, rounded once to fp32.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstring>
+
+#include "bard_internal.h"
+
+namespace bard {
+
+namespace {
+
+struct M3 { double m[9]; };
+struct V3 { double v[3]; };
+
+M3 mul(const M3& a, const M3& b) {
+  M3 c;
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j) {
+      double s = 0;
+      for (int k = 0; k < 3; ++k) s += a.m[3 * i + k] * b.m[3 * k + j];
+      c.m[3 * i + j] = s;
+    }
+  return c;
+}
+V3 mul(const M3& a, const V3& x) {
+  V3 y;
+  for (int i = 0; i < 3; ++i) y.v[i] = a.m[3 * i] * x.v[0] + a.m[3 * i + 1] * x.v[1] + a.m[3 * i + 2] * x.v[2];
+  return y;
+}
+M3 transpose(const M3& a) {
+  M3 c;
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j) c.m[3 * i + j] = a.m[3 * j + i];
+  return c;
+}
+M3 hat(const V3& k) {  // [k]x
+  M3 c = {{0, -k.v[2], k.v[1], k.v[2], 0, -k.v[0], -k.v[1], k.v[0], 0}};
+  return c;
+}
+V3 cross(const V3& a, const V3& b) {
+  V3 c = {{a.v[1] * b.v[2] - a.v[2] * b.v[1], a.v[2] * b.v[0] - a.v[0] * b.v[2], a.v[0] * b.v[1] - a.v[1] * b.v[0]}};
+  return c;
+}
+void split12(const double* T, M3& R, V3& t) {
+  for (int i = 0; i < 3; ++i) {
+    for (int j = 0; j < 3; ++j) R.m[3 * i + j] = T[4 * i + j];
+    t.v[i] = T[4 * i + 3];
+  }
+}
+bool is_identity12(const double* T) {
+  static const double I[12] = {1, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, 0};
+  for (int k = 0; k < 12; ++k)
+    if (std::fabs(T[k] - I[k]) > 1e-12) return false;
+  return true;
+}
+void put(float* dst, const double* src, int n) {
+  for (int k = 0; k < n; ++k) dst[k] = (float)src[k];
+}
+
+}  // namespace
+
+bard_status build_model(const bard_model_desc* d, int device, Model& M) {
+  if (!d || d->nb < 1 || !d->parent || !d->joint_type || !d->T_pre || !d->mass || !d->com || !d->inertia) {
+    set_error("bard_model_create: NULL pointer in description or nb < 1");
+    return BARD_ERR_INVALID_ARG;
+  }
+  const int nb = d->nb;
+  if (nb > BARD_MAX_BODIES) {
+    set_error("bard_model_create: nb exceeds BARD_MAX_BODIES");
+    return BARD_ERR_UNSUPPORTED;
+  }
+  for (int i = 0; i < nb; ++i) {
+    int t = d->joint_type[i];
+    if (t < 0 || t > 3) { set_error("bard_model_create: unknown joint type"); return BARD_ERR_INVALID_ARG; }
+    if (d->parent[i] >= i || d->parent[i] < -1) {
+      set_error("bard_model_create: parent[i] must be in {-1, 0..i-1}");
+      return BARD_ERR_TOPOLOGY;
+    }
+    if (!(d->mass[i] > 0.0)) { set_error("bard_model_create: mass must be positive"); return BARD_ERR_INVALID_ARG; }
+    if ((t == BARD_JOINT_REVOLUTE || t == BARD_JOINT_PRISMATIC)) {
+      if (!d->axis) { set_error("bard_model_create: axis is NULL"); return BARD_ERR_INVALID_ARG; }
+      const double* a = d->axis + 3 * i;
+      if (std::sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]) < 1e-12) {
+        set_error("bard_model_create: zero-length joint axis");
+        return BARD_ERR_INVALID_ARG;
+      }
+    }
+    if (t == BARD_JOINT_FREE && d->T_post && !is_identity12(d->T_post + 12 * i)) {
+      set_error("bard_model_create: T_post must be identity on a free joint");
+      return BARD_ERR_INVALID_ARG;
+    }
+  }
+  M.device = device;
+  M.nb = nb;
+  M.parent.assign(d->parent, d->parent + nb);
+  M.jtype.assign(d->joint_type, d->joint_type + nb);
+
+  // offsets
+  static const int NQ[4] = {1, 1, 0, 7}, NV[4] = {1, 1, 0, 6};
+  M.q_off.assign(nb + 1, 0);
+  M.v_off.assign(nb + 1, 0);
+  for (int i = 0; i < nb; ++i) {
+    M.q_off[i + 1] = M.q_off[i] + NQ[M.jtype[i]];
+    M.v_off[i + 1] = M.v_off[i] + NV[M.jtype[i]];
+  }
+  M.nq = M.q_off[nb];
+  M.nv = M.v_off[nb];
+  if (M.nv > BARD_MAX_DOF) { set_error("bard_model_create: nv exceeds BARD_MAX_DOF"); return BARD_ERR_UNSUPPORTED; }
+  M.dof_body.clear();
+  for (int i = 0; i < nb; ++i)
+    for (int k = 0; k < NV[M.jtype[i]]; ++k) M.dof_body.push_back(i);
+
+  // level schedule: level 0 = attached to world; inside a level ascending body index
+  M.body_level.assign(nb, 0);
+  int nl = 0;
+  for (int i = 0; i < nb; ++i) {
+    M.body_level[i] = M.parent[i] < 0 ? 0 : M.body_level[M.parent[i]] + 1;
+    if (M.body_level[i] + 1 > nl) nl = M.body_level[i] + 1;
+  }
+  M.nlevels = nl;
+  M.level_ptr.assign(nl + 1, 0);
+  for (int i = 0; i < nb; ++i) M.level_ptr[M.body_level[i] + 1]++;
+  for (int l = 0; l < nl; ++l) M.level_ptr[l + 1] += M.level_ptr[l];
+  M.level_body.assign(nb, 0);
+  std::vector<int32_t> slot_of(nb, -1), cursor(M.level_ptr.begin(), M.level_ptr.end() - 1);
+  for (int i = 0; i < nb; ++i) {
+    int s = cursor[M.body_level[i]]++;
+    M.level_body[s] = i;
+    slot_of[i] = s;
+  }
+  M.parent_slot.assign(nb, -1);
+  for (int s = 0; s < nb; ++s) {
+    int p = M.parent[M.level_body[s]];
+    M.parent_slot[s] = p < 0 ? -1 : slot_of[p];
+  }
+  M.anc_mask.assign(nb, 0);
+  for (int i = 0; i < nb; ++i) M.anc_mask[i] = (1ull << i) | (M.parent[i] < 0 ? 0ull : M.anc_mask[M.parent[i]]);
+
+  // Slots for the outward sweeps (thread-per-env kernels walk bodies in index order): a body whose
+  // children are not all "the next body" parks its state in a slot until its last child has read it.
+  std::vector<int32_t> last_child(nb, -1), save(nb, -1), src(nb, -1);
+  std::vector<char> needs(nb, 0);
+  for (int i = 0; i < nb; ++i) {
+    int p = M.parent[i];
+    if (p >= 0) {
+      if (p != i - 1) needs[p] = 1;
+      last_child[p] = i;
+    }
+  }
+  std::vector<int32_t> free_list;
+  int nslots = 0;
+  std::vector<std::vector<int32_t>> release_at(nb + 1);
+  for (int i = 0; i < nb; ++i) {
+    int p = M.parent[i];
+    src[i] = p < 0 ? -1 : (p == i - 1 ? -2 : save[p]);
+    for (int s : release_at[i]) free_list.push_back(s);   // slots whose last reader was body i-1... see below
+    if (needs[i]) {
+      int s;
+      if (!free_list.empty()) { s = free_list.back(); free_list.pop_back(); }
+      else s = nslots++;
+      save[i] = s;
+      release_at[last_child[i] + 1].push_back(s);
+    }
+  }
+  M.nslots = nslots;
+
+  // constant blob
+  M.blob_bytes = sizeof(BlobHeader) + sizeof(BodyConst) * nb + sizeof(FrameConst) * BARD_MAX_FRAMES;
+  M.blob.assign(M.blob_bytes, 0);
+  BlobHeader* H = reinterpret_cast<BlobHeader*>(M.blob.data());
+  H->nb = nb; H->nq = M.nq; H->nv = M.nv; H->nlevels = nl; H->nslots = nslots; H->nframes = 0;
+  for (int k = 0; k < 3; ++k) H->g[k] = (float)d->gravity[k];
+  BodyConst* BC = reinterpret_cast<BodyConst*>(M.blob.data() + sizeof(BlobHeader));
+  M.rodrigues.assign((size_t)nb * 36, 0.f);
+  for (int i = 0; i < nb; ++i) {
+    BodyConst& c = BC[i];
+    const int t = M.jtype[i];
+    M3 Rpre, Rpost = {{1, 0, 0, 0, 1, 0, 0, 0, 1}};
+    V3 tpre, tpost = {{0, 0, 0}};
+    split12(d->T_pre + 12 * i, Rpre, tpre);
+    bool post_id = true;
+    if (d->T_post) { split12(d->T_post + 12 * i, Rpost, tpost); post_id = is_identity12(d->T_post + 12 * i); }
+    V3 ax = {{0, 0, 0}};
+    if (t == BARD_JOINT_REVOLUTE || t == BARD_JOINT_PRISMATIC) {
+      const double* a = d->axis + 3 * i;
+      double n = std::sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]);
+      for (int k = 0; k < 3; ++k) ax.v[k] = a[k] / n;
+    }
+    double rod[36];
+    std::memset(rod, 0, sizeof(rod));
+    M3 R0 = mul(Rpre, Rpost);
+    V3 t0 = mul(Rpre, tpost);
+    for (int k = 0; k < 3; ++k) t0.v[k] += tpre.v[k];
+    std::memcpy(rod, R0.m, sizeof(R0.m));
+    std::memcpy(rod + 27, t0.v, sizeof(t0.v));
+    double Sw[3] = {0, 0, 0}, Sl[3] = {0, 0, 0};
+    if (t == BARD_JOINT_REVOLUTE) {
+      M3 K = hat(ax), K2 = mul(K, K);
+      M3 RK = mul(Rpre, K), RK2 = mul(Rpre, K2);
+      M3 A = mul(RK, Rpost), Bm = mul(RK2, Rpost);
+      V3 a = mul(RK, tpost), b = mul(RK2, tpost);
+      std::memcpy(rod + 9, A.m, sizeof(A.m));
+      std::memcpy(rod + 18, Bm.m, sizeof(Bm.m));
+      std::memcpy(rod + 30, a.v, sizeof(a.v));
+      std::memcpy(rod + 33, b.v, sizeof(b.v));
+      // S = X_post^{-1} [axis; 0] in the body frame: w = Rpost^T axis, l = Rpost^T (axis x tpost)
+      M3 Rt = transpose(Rpost);
+      V3 w = mul(Rt, ax), l = mul(Rt, cross(ax, tpost));
+      for (int k = 0; k < 3; ++k) { Sw[k] = w.v[k]; Sl[k] = l.v[k]; }
+    } else if (t == BARD_JOINT_PRISMATIC) {
+      V3 a = mul(Rpre, ax);
+      std::memcpy(rod + 30, a.v, sizeof(a.v));
+      V3 l = mul(transpose(Rpost), ax);
+      for (int k = 0; k < 3; ++k) Sl[k] = l.v[k];
+    } else if (t == BARD_JOINT_FREE) {
+      std::memcpy(rod, Rpre.m, sizeof(Rpre.m));
+      std::memcpy(rod + 27, tpre.v, sizeof(tpre.v));
+    }
+    put(c.R0, rod, 36);
+    put(&M.rodrigues[(size_t)36 * i], rod, 36);
+    put(c.Sw, Sw, 3);
+    put(c.Sl, Sl, 3);
+    // compact spatial inertia about the body origin: m, h = m c, Io = Ic + m (|c|^2 1 - c c^T)
+    const double m = d->mass[i];
+    const double* cm = d->com + 3 * i;
+    const double* Ic = d->inertia + 6 * i;
+    const double c2 = cm[0] * cm[0] + cm[1] * cm[1] + cm[2] * cm[2];
+    double Io[6] = {Ic[0] + m * (c2 - cm[0] * cm[0]), Ic[1] - m * cm[0] * cm[1], Ic[2] - m * cm[0] * cm[2],
+                    Ic[3] + m * (c2 - cm[1] * cm[1]), Ic[4] - m * cm[1] * cm[2], Ic[5] + m * (c2 - cm[2] * cm[2])};
+    double h[3] = {m * cm[0], m * cm[1], m * cm[2]};
+    c.mass = (float)m;
+    put(c.h, h, 3);
+    put(c.Io, Io, 6);
+    c.type = t; c.parent = M.parent[i]; c.q_off = M.q_off[i]; c.v_off = M.v_off[i];
+    c.src = src[i]; c.save = save[i]; c.flags = post_id ? 1 : 0; c.level = M.body_level[i];
+    c.anc_lo = (uint32_t)M.anc_mask[i]; c.anc_hi = (uint32_t)(M.anc_mask[i] >> 32);
+  }
+
+  if (device < 0) return BARD_OK;  // host-only model: tables can be queried, operators refuse to run
+  int dev_count = 0;
+  cudaError_t e = cudaGetDeviceCount(&dev_count);
+  if (e != cudaSuccess || device < 0 || device >= dev_count) {
+    set_error(std::string("bard_model_create: no such CUDA device: ") + cudaGetErrorString(e));
+    cudaGetLastError();
+    return BARD_ERR_CUDA;
+  }
+  int prev = 0;
+  cudaGetDevice(&prev);
+  cudaSetDevice(device);
+  cudaDeviceGetAttribute(&M.sm_count, cudaDevAttrMultiProcessorCount, device);
+  e = cudaMalloc(&M.d_blob, M.blob_bytes);
+  if (e == cudaSuccess) e = cudaMemcpy(M.d_blob, M.blob.data(), M.blob_bytes, cudaMemcpyHostToDevice);
+  cudaSetDevice(prev);
+  if (e != cudaSuccess) {
+    set_error(std::string("bard_model_create: ") + cudaGetErrorString(e));
+    if (M.d_blob) cudaFree(M.d_blob);
+    M.d_blob = nullptr;
+    return e == cudaErrorMemoryAllocation ? BARD_ERR_ALLOC : BARD_ERR_CUDA;
+  }
+  return BARD_OK;
+}
+
+bard_status set_frames(Model& M, int32_t nframes, const int32_t* body, const double* offset) {
+  if (nframes < 0 || (nframes > 0 && !body)) { set_error("bard_model_set_frames: bad arguments"); return BARD_ERR_INVALID_ARG; }
+  if (nframes > BARD_MAX_FRAMES) { set_error("bard_model_set_frames: too many frames"); return BARD_ERR_UNSUPPORTED; }
+  for (int f = 0; f < nframes; ++f)
+    if (body[f] < 0 || body[f] >= M.nb) { set_error("bard_model_set_frames: frame body out of range"); return BARD_ERR_INVALID_ARG; }
+  BlobHeader* H = reinterpret_cast<BlobHeader*>(M.blob.data());
+  FrameConst* F = reinterpret_cast<FrameConst*>(M.blob.data() + sizeof(BlobHeader) + sizeof(BodyConst) * M.nb);
+  uint64_t uni = 0;
+  std::memset(F, 0, sizeof(FrameConst) * BARD_MAX_FRAMES);
+  for (int f = 0; f < nframes; ++f) {
+    F[f].body = body[f];
+    for (int k = 0; k < 3; ++k) F[f].off[k] = offset ? (float)offset[3 * f + k] : 0.f;
+    uint64_t a = M.anc_mask[body[f]];
+    F[f].anc_lo = (uint32_t)a; F[f].anc_hi = (uint32_t)(a >> 32);
+    uni |= a;
+  }
+  H->nframes = nframes;
+  H->jac_mask_lo = (int32_t)(uint32_t)uni; H->jac_mask_hi = (int32_t)(uint32_t)(uni >> 32);
+  M.nframes = nframes;
+  if (!M.d_blob) return BARD_OK;
+  int prev = 0;
+  cudaGetDevice(&prev);
+  cudaSetDevice(M.device);
+  cudaError_t e = cudaMemcpy(M.d_blob, M.blob.data(), M.blob_bytes, cudaMemcpyHostToDevice);
+  cudaSetDevice(prev);
+  if (e != cudaSuccess) { set_error(std::string("bard_model_set_frames: ") + cudaGetErrorString(e)); return BARD_ERR_CUDA; }
+  return BARD_OK;
+}
+
+}  // namespace bard
