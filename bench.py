@@ -1,0 +1,396 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the batched rigid-body hot path (FK, Jacobian, RNEA, CRBA) on B200.
+
+A "step" is one pass of the whole hot path over one batch of synthetic states: bard_fk, bard_jacobian,
+bard_rnea and bard_crba (four kernel launches through the C ABI) on B environments.  One "env-eval" is all
+four operators evaluated for one environment.  Default workload: config 3 (23-DOF humanoid) at B = 65 536,
+the point of BASELINE.json's sweep (config 4) from which north_star's roofline target applies.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0..3] [--B n] [--impl ours|reference]
+
+Multi-GPU (N > 1, under torch.distributed.run): the batch axis shards, every rank evaluates its own B
+environments with a replicated model and no data-path collective -> "scaling": "weak".
+
+``--impl reference`` times the fp64 CPU oracle (oracle/, test infrastructure) on a bounded sample of the
+same workload on the host cores; rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2605_31481_b200 import roofline as RL            # noqa: E402
+from paper_2605_31481_b200 import workloads as W            # noqa: E402
+
+OPS = ("fk", "jacobian", "rnea", "crba")
+METRIC = "env_evals_per_s (FK + Jacobian + RNEA + CRBA per environment)"
+UNIT = "env-evals/s"
+L2_BYTES = 126 * 1024 * 1024
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=300)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--config", type=int, default=3, choices=[0, 1, 2, 3])
+    ap.add_argument("--B", type=int, default=65536)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--sweep", action="store_true", help="also time every operator over config 4's batch sweep")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU work for the oracle baseline")
+    return ap.parse_args()
+
+
+def workload_name(cfg, B):
+    return f"config{cfg}:{W.CONFIG_NAMES[cfg]} B={B} (sweep point of config 4)"
+
+
+# --------------------------------------------------------------------------------------- oracle timing
+def time_oracle(desc, cfg, seconds):
+    """The fp64 oracle as it stands, all four operators, OpenMP over environments on the host cores, on a
+    bounded sample of the workload's states (same seeded distributions).  Returns env-evals/s and details."""
+    import oracle
+    o = oracle.Oracle(desc)
+    cores = os.cpu_count() or 1
+    oracle.set_threads(cores)
+    used = oracle.get_threads()
+
+    def one_pass(q, qd, qdd):
+        t0 = time.perf_counter()
+        o.fk(q)
+        o.jacobian(q)
+        o.rnea(q, qd, qdd)
+        o.crba(q)
+        return time.perf_counter() - t0
+
+    n0 = 2048
+    q, qd, qdd = (a.astype(np.float64) for a in W.config_states(cfg, n0))
+    one_pass(q, qd, qdd)                                  # warm pass (page-in, thread pool)
+    t = one_pass(q, qd, qdd)
+    n = int(min(262144, max(n0, n0 * (seconds / 3.0) / max(t, 1e-6))))
+    q, qd, qdd = (a.astype(np.float64) for a in W.config_states(cfg, n))
+    best = min(one_pass(q, qd, qdd) for _ in range(3))
+    return {"value": n / best, "unit": UNIT, "cores": used, "kind": "oracle",
+            "sample": f"{n} environments of the workload's seeded state distribution, all four operators, "
+                      f"fp64, best of 3 passes ({best:.3f} s per pass)"}, n, best
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    desc = W.config_robot(args.config)
+    import oracle
+    o = oracle.Oracle(desc)
+    oracle.set_threads(os.cpu_count() or 1)
+    n = 8192                                             # bounded sample per step
+    q, qd, qdd = (a.astype(np.float64) for a in W.config_states(args.config, n))
+
+    def step():
+        o.fk(q); o.jacobian(q); o.rnea(q, qd, qdd); o.crba(q)
+
+    steps = min(args.steps, 20)
+    warm = min(args.warmup, 3)
+    for _ in range(warm):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        step()
+    dt = time.perf_counter() - t0
+    val = n * steps / dt
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+        "warmup": warm, "ms_per_step": 1e3 * dt / steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(args.config, args.B),
+                   "note": f"oracle timed on a bounded sample of {n} environments per step (host cores)"},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": oracle.get_threads(), "kind": "oracle",
+                         "sample": f"{n} environments per step x {steps} steps"},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# --------------------------------------------------------------------------------------- clocks sampler
+class Clocks(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed regions run."""
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap"}
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.samples, self.reasons, self.max_mhz, self.ok = [], set(), None, False
+        self._stop_evt = threading.Event()
+        self.active = threading.Event()
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        while not self._stop_evt.is_set():
+            if self.active.is_set():
+                try:
+                    self.samples.append(float(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM)))
+                    r = int(self.nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                    for bit, name in self.REASONS.items():
+                        if r & bit:
+                            self.reasons.add(name)
+                except Exception:
+                    pass
+            time.sleep(0.005)
+
+    def stop(self):
+        self._stop_evt.set()
+
+    def summary(self):
+        if not self.ok or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": 0}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# --------------------------------------------------------------------------------------- our arm
+class BufferSet:
+    """One set of device inputs and outputs (SoA, batch last) for B environments."""
+
+    def __init__(self, torch, m, desc, cfg, B, seed_step, dev):
+        q, qd, qdd = W.sample_states(desc, B, seed=2000 + cfg + 100 * seed_step)
+        self.q, self.qd, self.qdd = (torch.from_numpy(a).to(dev) for a in (q, qd, qdd))
+        self.pose = torch.empty((m.nb, 12, B), device=dev)
+        self.J = torch.empty((m.nframes, 6, m.nv, B), device=dev)
+        self.tau = torch.empty((m.nv, B), device=dev)
+        self.M = torch.empty((m.nv, m.nv, B), device=dev)
+
+    def nbytes(self):
+        return sum(t.numel() * 4 for t in (self.q, self.qd, self.qdd, self.pose, self.J, self.tau, self.M))
+
+
+def op_call(m, op, s, B, stream):
+    if op == "fk":
+        m.fk(B, s.q, s.pose, stream)
+    elif op == "jacobian":
+        m.jacobian(B, s.q, s.J, stream)
+    elif op == "rnea":
+        m.rnea(B, s.q, s.qd, s.qdd, s.tau, stream)
+    else:
+        m.crba(B, s.q, s.M, stream)
+
+
+def make_sets(torch, m, desc, cfg, B, dev, min_sets=3, cap_bytes=48 << 30):
+    first = BufferSet(torch, m, desc, cfg, B, 0, dev)
+    per = first.nbytes()
+    n = max(min_sets, -(-3 * L2_BYTES // per))           # rotating sets: total >= 3 x L2
+    n = max(1, min(n, cap_bytes // per))
+    return [first] + [BufferSet(torch, m, desc, cfg, B, i, dev) for i in range(1, n)], per
+
+
+def time_op_train(torch, m, op, sets, B, stream, launches, warm=5):
+    """Average duration of one launch of `op`, back to back over rotating buffer sets, CUDA events on `stream`."""
+    for i in range(warm):
+        op_call(m, op, sets[i % len(sets)], B, stream)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for i in range(launches):
+        op_call(m, op, sets[i % len(sets)], B, stream)
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) * 1e-3 / launches
+
+
+def op_report(desc, pk, op, sec, B):
+    r = RL.roofline(desc, pk)[op]
+    if r["bound"] == "hbm":
+        ach, peak, unit = r["bytes"] * B / sec / 1e9, pk["hbm_gbs"], "GB/s"
+    else:
+        ach, peak, unit = r["flop"] * B / sec / 1e12, pk["fp32_tflops"], "TFLOP/s"
+    return {"us": sec * 1e6, "env_evals_per_s": B / sec, "bound": r["bound"], "achieved": ach, "peak": peak,
+            "unit": unit, "frac": ach / peak, "bytes_per_env": r["bytes"], "flop_per_env": r["flop"],
+            "hbm_gbs": r["bytes"] * B / sec / 1e9, "fp32_tflops": r["flop"] * B / sec / 1e12}
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2605_31481_b200 import binding
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg, B, K, Wm = args.config, args.B, args.steps, max(args.warmup, 3)
+    desc = W.config_robot(cfg)
+    m = binding.Model(desc, device=local)
+    pk = RL.measured_peaks(ROOT)
+    sets, per_set = make_sets(torch, m, desc, cfg, B, dev)
+    R = len(sets)
+    stream = torch.cuda.current_stream().cuda_stream
+    clocks = Clocks(local)
+    clocks.start()
+
+    def step(i, ev=None):
+        s = sets[i % R]
+        for k, op in enumerate(OPS):
+            if ev is not None:
+                ev[k].record()
+            op_call(m, op, s, B, stream)
+        if ev is not None:
+            ev[4].record()
+
+    # ---- device-resident timed region: W warm-up steps, then exactly K steps
+    for i in range(Wm):
+        step(i)
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(K)]
+    barrier()
+    clocks.active.set()
+    n0 = binding.launch_count()
+    for i in range(K):
+        step(i, evs[i])
+    barrier()
+    clocks.active.clear()
+    launches = binding.launch_count() - n0
+    elapsed_ms = evs[0][0].elapsed_time(evs[-1][4])
+    t = torch.tensor([elapsed_ms], device=dev, dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    elapsed_ms = float(t.item())
+    value = world * B * K / (elapsed_ms * 1e-3)
+    op_sec = {op: float(np.mean([evs[i][k].elapsed_time(evs[i][k + 1]) for i in range(K)])) * 1e-3
+              for k, op in enumerate(OPS)}
+    ops = {op: op_report(desc, pk, op, op_sec[op], B) for op in OPS}
+    for op in OPS:
+        ops[op]["share_of_step"] = op_sec[op] / sum(op_sec.values())
+
+    # ---- per-operator back-to-back trains (no events between launches), same rotating buffers
+    clocks.active.set()
+    for op in OPS:
+        sec = time_op_train(torch, m, op, sets, B, stream, launches=max(50, min(K, 500)))
+        ops[op]["train"] = {k: v for k, v in op_report(desc, pk, op, sec, B).items()
+                            if k in ("us", "env_evals_per_s", "achieved", "frac", "hbm_gbs", "fp32_tflops")}
+    clocks.active.clear()
+
+    # ---- end to end: pinned host inputs -> device, four launches, every output -> pinned host, per step
+    s0 = sets[0]
+    h_in = [torch.empty(x.shape, dtype=x.dtype, pin_memory=True).copy_(x.cpu()) for x in (s0.q, s0.qd, s0.qdd)]
+    d_out = (s0.pose, s0.J, s0.tau, s0.M)
+    h_out = [torch.empty(x.shape, dtype=x.dtype, pin_memory=True) for x in d_out]
+    h2d = sum(x.numel() * 4 for x in h_in)
+    d2h = sum(x.numel() * 4 for x in h_out)
+    Ke = max(3, min(K, 20))
+
+    def e2e_step():
+        for h, d in zip(h_in, (s0.q, s0.qd, s0.qdd)):
+            d.copy_(h, non_blocking=True)
+        for op in OPS:
+            op_call(m, op, s0, B, stream)
+        for h, d in zip(h_out, d_out):
+            h.copy_(d, non_blocking=True)
+        torch.cuda.current_stream().synchronize()       # the caller reads the results on the host
+
+    for _ in range(2):
+        e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(Ke):
+        e2e_step()
+    barrier()
+    te = torch.tensor([time.perf_counter() - t0], device=dev, dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e = {"value": world * B * Ke / float(te.item()), "unit": UNIT, "h2d_bytes_per_step": h2d,
+           "d2h_bytes_per_step": d2h, "steps": Ke,
+           "note": "pinned host q/qd/qdd -> device, 4 launches, pose/J/tau/M -> pinned host, every step"}
+    clocks.stop()
+
+    dom = max(OPS, key=lambda o: op_sec[o])
+    d = ops[dom]
+    roof = {"kernel": f"{dom}_kernel", "bound": d["bound"], "achieved": d["achieved"], "peak": d["peak"],
+            "unit": d["unit"], "frac": d["frac"], "traffic": None,
+            "peak_source": ("MEASURED_PEAKS.json hbm_gbs" if d["bound"] == "hbm" else
+                            "derived: 148 SM x 128 lanes x 2 x sm_max_mhz") + f" ({pk['source']})",
+            "algorithmic_per_launch": (d["bytes_per_env"] if d["bound"] == "hbm" else d["flop_per_env"]) * B,
+            "avg_launch_us": d["us"]}
+    tr = os.path.join(ROOT, "profiles", "traffic.json")   # dram bytes per launch from the committed ncu capture
+    if os.path.exists(tr):
+        try:
+            roof["traffic"] = json.load(open(tr)).get(f"config{cfg}_B{B}", {}).get(dom)
+        except Exception:
+            pass
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+        "ms_per_step": elapsed_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": workload_name(cfg, B), "envs_per_gpu": B, "global_envs": world * B,
+                   "parallelism": f"batch-sharded x{world}, no collective",
+                   "l2": f"{R} rotating buffer sets of {per_set / 1e6:.1f} MB (total {R * per_set / 1e6:.0f} MB > L2 126 MB)",
+                   "layout": "SoA batch-fastest"},
+        "roofline": roof, "ops": ops, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks.summary(),
+    }
+    if args.sweep and rank == 0:
+        line["sweep"] = sweep(torch, binding, pk, dev, stream)
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cb, _, _ = time_oracle(desc, cfg, args.cpu_seconds)
+        line["cpu_baseline"] = cb
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def sweep(torch, binding, pk, dev, stream):
+    """config 4: every operator on the humanoid and the chain at B = 1024 ... 1 048 576 (train timing)."""
+    out = {}
+    for cfg in (3, 0):
+        desc = W.config_robot(cfg)
+        m = binding.Model(desc, device=dev.index or 0)
+        for B in (1024, 4096, 16384, 65536, 262144, 1048576):
+            sets, _ = make_sets(torch, m, desc, cfg, B, dev, cap_bytes=40 << 30)
+            row = {}
+            for op in OPS:
+                sec = time_op_train(torch, m, op, sets, B, stream, launches=100)
+                r = op_report(desc, pk, op, sec, B)
+                row[op] = {k: r[k] for k in ("us", "env_evals_per_s", "bound", "frac", "hbm_gbs", "fp32_tflops")}
+            out[f"{W.CONFIG_NAMES[cfg]}_B{B}"] = row
+            del sets
+            torch.cuda.empty_cache()
+        m.close()
+    return out
+
+
+if __name__ == "__main__":
+    a = parse()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)
