@@ -103,9 +103,9 @@ bard_status bard_fk(const bard_model* bm, int64_t B, const float* q, float* pose
 }
 
 bard_status bard_jacobian(const bard_model* bm, int64_t B, const float* q, float* J, bard_stream stream) {
-  bard_status s = check_call("bard_jacobian", bm, B, bm && bm->m.nq == 0 ? (const void*)J : q, J, J, J);
+  if (bm && (bm->m.nframes == 0 || bm->m.nv == 0)) return check_call("bard_jacobian", bm, B, bm, bm, bm, bm);  // empty output
+  bard_status s = check_call("bard_jacobian", bm, B, bm->m.nq == 0 ? (const void*)J : q, J, J, J);
   if (s != BARD_OK || B == 0) return s;
-  if (bm->m.nframes == 0 || bm->m.nv == 0) return BARD_OK;  // empty output
   return bard::launch_jacobian(bm->m, B, q, J, stream);
 }
 

@@ -28,12 +28,14 @@ struct BodyConst {
   int32_t type;               // 52
   int32_t parent;             // 53
   int32_t q_off, v_off;       // 54, 55
-  int32_t src;                // 56  where the parent's state is: -1 world, -2 the previous body (registers), >=0 slot
-  int32_t save;               // 57  slot this body's state is saved to for later children (-1: none)
+  int32_t src;                // 56  where the parent's state is: -1 world, -2 registers of the same warp
+                              //     (the task this warp processed just before), >=0 shared-memory slot
+  int32_t save;               // 57  slot this body's state is saved to for children on other warps (-1: none)
   int32_t flags;              // 58  bit0: T_post is identity (a = b = 0, Sl = 0)
   int32_t level;              // 59
   uint32_t anc_lo, anc_hi;    // 60, 61  ancestor-or-self mask of this body
-  int32_t pad[2];             // 62, 63
+  int32_t child_begin;        // 62  first entry of this body's children in the CHILDREN table
+  int32_t child_count;        // 63
 };
 static_assert(sizeof(BodyConst) == 256, "BodyConst must be 64 words");
 
@@ -44,20 +46,37 @@ struct FrameConst {           // 8 words
   int32_t pad[2];
 };
 
-// Header of the device blob; followed by BodyConst[nb], then FrameConst[BARD_MAX_FRAMES].
-struct BlobHeader {           // 16 words
+// Level-parallel schedule (eq. (6)): one TEAM of `team_warps` warps evaluates 32
+// environments (lane = environment).  Bodies of one tree level are spread over the team's warps; the warps
+// meet at a named barrier between levels.  Every warp walks its own flat task list
+//   task = body | TASK_BAR (team barrier after this task) | TASK_NOOP (no body: barrier only)
+// terminated by TASK_END; the inward sweeps of RNEA / CRBA walk the same list backwards.
+enum : uint16_t { TASK_BODY_MASK = 0x00ff, TASK_BAR = 0x0100, TASK_NOOP = 0x0200, TASK_END = 0xffff };
+
+// Header of the device blob; followed by BodyConst[nb], FrameConst[BARD_MAX_FRAMES], then the schedule
+// tables at the byte offsets stored here (each 16-byte aligned).
+struct BlobHeader {           // 32 words
   int32_t nb, nq, nv, nlevels;
   int32_t nslots;             // number of parent-state slots the outward sweeps need
   int32_t nframes;
   int32_t jac_mask_lo, jac_mask_hi;  // union of the frames' ancestor masks
   float   g[3];               // gravity, world
-  int32_t pad[5];
+  int32_t team_warps;         // L
+  int32_t off_tasks;          // uint16 [team_warps][task_stride]
+  int32_t task_stride;
+  int32_t off_children;       // uint8 [nb]: children lists, ascending, concatenated in body order
+  int32_t off_fill;           // uint8 [team_warps][fill_stride]: DOFs (rows of M) each warp fills, 0xff ends
+  int32_t fill_stride;
+  int32_t off_dof_body;       // uint8 [nv]
+  int32_t pad[14];
 };
-static_assert(sizeof(BlobHeader) == 64, "BlobHeader must be 16 words");
+static_assert(sizeof(BlobHeader) == 128, "BlobHeader must be 32 words");
 
 struct Model {
   int device = 0;
   int32_t nb = 0, nq = 0, nv = 0, nlevels = 0, nslots = 0, nframes = 0;
+  int32_t team_warps = 1;             // L: warps that share one 32-environment tile (level-parallel schedule)
+  std::vector<int32_t> warp_of;       // body -> warp of its team
   std::vector<int32_t> parent, jtype, level_ptr, level_body, body_level, parent_slot, q_off, v_off, dof_body;
   std::vector<uint64_t> anc_mask;
   std::vector<float> rodrigues;       // nb*36

@@ -3,7 +3,9 @@
 // outward sweeps, and the single upload of the constant blob.  All precompute is fp64, rounded once to fp32.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 
 #include "bard_internal.h"
@@ -139,40 +141,124 @@ bard_status build_model(const bard_model_desc* d, int device, Model& M) {
   M.anc_mask.assign(nb, 0);
   for (int i = 0; i < nb; ++i) M.anc_mask[i] = (1ull << i) | (M.parent[i] < 0 ? 0ull : M.anc_mask[M.parent[i]]);
 
-  // Slots for the outward sweeps (thread-per-env kernels walk bodies in index order): a body whose
-  // children are not all "the next body" parks its state in a slot until its last child has read it.
-  std::vector<int32_t> last_child(nb, -1), save(nb, -1), src(nb, -1);
-  std::vector<char> needs(nb, 0);
-  for (int i = 0; i < nb; ++i) {
-    int p = M.parent[i];
-    if (p >= 0) {
-      if (p != i - 1) needs[p] = 1;
-      last_child[p] = i;
+  // ---- level-parallel team schedule: L warps share one 32-environment tile.
+  std::vector<std::vector<int32_t>> children(nb);
+  for (int i = 0; i < nb; ++i)
+    if (M.parent[i] >= 0) children[M.parent[i]].push_back(i);
+  int maxw = 1;
+  for (int l = 0; l < nl; ++l) maxw = std::max(maxw, (int)(M.level_ptr[l + 1] - M.level_ptr[l]));
+  int L = std::min(maxw, 8);
+  if (const char* ev = std::getenv("BARD_TEAM_WARPS")) {   // tuning knob for experiments
+    int v = std::atoi(ev);
+    if (v >= 1 && v <= 8) L = v;
+  }
+  M.team_warps = L;
+  // Bodies of a level go to warps: a body continues on its parent's warp when the parent was that warp's
+  // last task (its state is then still in registers); the others go to the least loaded warp.
+  M.warp_of.assign(nb, 0);
+  std::vector<std::vector<uint16_t>> tasks(L);
+  std::vector<int32_t> last_task(L, -1), total(L, 0), src(nb, -1), save(nb, -1);
+  std::vector<char> reg_fed(nb, 0);
+  for (int l = 0; l < nl; ++l) {
+    std::vector<std::vector<int32_t>> mine(L);
+    std::vector<int32_t> load(L, 0);
+    std::vector<char> claimed(L, 0), placed(nb, 0);
+    for (int s = M.level_ptr[l]; s < M.level_ptr[l + 1]; ++s) {
+      const int b = M.level_body[s], p = M.parent[b];
+      if (p < 0) continue;
+      const int w = M.warp_of[p];
+      if (last_task[w] == p && !claimed[w]) {
+        claimed[w] = 1; placed[b] = 1; reg_fed[b] = 1;
+        M.warp_of[b] = w; mine[w].push_back(b); load[w]++;
+      }
+    }
+    for (int s = M.level_ptr[l]; s < M.level_ptr[l + 1]; ++s) {
+      const int b = M.level_body[s];
+      if (placed[b]) continue;
+      int best = 0;
+      for (int w = 1; w < L; ++w)
+        if (load[w] < load[best] || (load[w] == load[best] && total[w] < total[best])) best = w;
+      M.warp_of[b] = best; mine[best].push_back(b); load[best]++;
+    }
+    for (int w = 0; w < L; ++w) {
+      if (mine[w].empty()) {
+        tasks[w].push_back((uint16_t)(TASK_NOOP | TASK_BAR));
+      } else {
+        for (size_t k = 0; k < mine[w].size(); ++k)
+          tasks[w].push_back((uint16_t)(mine[w][k] | (k + 1 == mine[w].size() ? TASK_BAR : 0)));
+        last_task[w] = mine[w].back();
+        total[w] += (int)mine[w].size();
+      }
     }
   }
-  std::vector<int32_t> free_list;
   int nslots = 0;
-  std::vector<std::vector<int32_t>> release_at(nb + 1);
   for (int i = 0; i < nb; ++i) {
-    int p = M.parent[i];
-    src[i] = p < 0 ? -1 : (p == i - 1 ? -2 : save[p]);
-    for (int s : release_at[i]) free_list.push_back(s);   // slots whose last reader was body i-1... see below
-    if (needs[i]) {
-      int s;
-      if (!free_list.empty()) { s = free_list.back(); free_list.pop_back(); }
-      else s = nslots++;
-      save[i] = s;
-      release_at[last_child[i] + 1].push_back(s);
+    bool need = false;
+    for (int c : children[i]) need = need || !reg_fed[c];
+    if (need) save[i] = nslots++;
+  }
+  for (int i = 0; i < nb; ++i) src[i] = M.parent[i] < 0 ? -1 : (reg_fed[i] ? -2 : save[M.parent[i]]);
+  M.nslots = nslots;
+  size_t task_stride = 0;
+  for (int w = 0; w < L; ++w) task_stride = std::max(task_stride, tasks[w].size() + 1);
+  task_stride = (task_stride + 7) & ~(size_t)7;
+  // rows of M (DOFs) each warp fills: longest-processing-time greedy on the row length i + 1
+  std::vector<std::vector<uint8_t>> fill(L);
+  {
+    std::vector<int64_t> work(L, 0);
+    for (int i = M.nv - 1; i >= 0; --i) {
+      int best = 0;
+      for (int w = 1; w < L; ++w)
+        if (work[w] < work[best]) best = w;
+      fill[best].push_back((uint8_t)i);
+      work[best] += i + 1;
     }
   }
-  M.nslots = nslots;
+  size_t fill_stride = 0;
+  for (int w = 0; w < L; ++w) fill_stride = std::max(fill_stride, fill[w].size() + 1);
+  fill_stride = (fill_stride + 15) & ~(size_t)15;
 
   // constant blob
-  M.blob_bytes = sizeof(BlobHeader) + sizeof(BodyConst) * nb + sizeof(FrameConst) * BARD_MAX_FRAMES;
+  auto align16 = [](size_t x) { return (x + 15) & ~(size_t)15; };
+  const size_t off_bodies = sizeof(BlobHeader);
+  const size_t off_frames = off_bodies + sizeof(BodyConst) * nb;
+  const size_t off_tasks = off_frames + sizeof(FrameConst) * BARD_MAX_FRAMES;
+  const size_t off_children = align16(off_tasks + sizeof(uint16_t) * L * task_stride);
+  const size_t off_fill = align16(off_children + (size_t)nb);
+  const size_t off_dof_body = align16(off_fill + (size_t)L * fill_stride);
+  M.blob_bytes = align16(off_dof_body + (size_t)M.nv);
   M.blob.assign(M.blob_bytes, 0);
   BlobHeader* H = reinterpret_cast<BlobHeader*>(M.blob.data());
   H->nb = nb; H->nq = M.nq; H->nv = M.nv; H->nlevels = nl; H->nslots = nslots; H->nframes = 0;
   for (int k = 0; k < 3; ++k) H->g[k] = (float)d->gravity[k];
+  H->team_warps = L;
+  H->off_tasks = (int32_t)off_tasks; H->task_stride = (int32_t)task_stride;
+  H->off_children = (int32_t)off_children;
+  H->off_fill = (int32_t)off_fill; H->fill_stride = (int32_t)fill_stride;
+  H->off_dof_body = (int32_t)off_dof_body;
+  {
+    uint16_t* T = reinterpret_cast<uint16_t*>(M.blob.data() + off_tasks);
+    for (int w = 0; w < L; ++w) {
+      for (size_t k = 0; k < task_stride; ++k) T[w * task_stride + k] = TASK_END;
+      for (size_t k = 0; k < tasks[w].size(); ++k) T[w * task_stride + k] = tasks[w][k];
+    }
+    uint8_t* F = M.blob.data() + off_fill;
+    for (int w = 0; w < L; ++w) {
+      for (size_t k = 0; k < fill_stride; ++k) F[w * fill_stride + k] = 0xff;
+      for (size_t k = 0; k < fill[w].size(); ++k) F[w * fill_stride + k] = fill[w][k];
+    }
+    uint8_t* D = M.blob.data() + off_dof_body;
+    for (int j = 0; j < M.nv; ++j) D[j] = (uint8_t)M.dof_body[j];
+  }
+  std::vector<int32_t> child_begin(nb, 0);
+  {
+    uint8_t* C = M.blob.data() + off_children;
+    int pos = 0;
+    for (int i = 0; i < nb; ++i) {
+      child_begin[i] = pos;
+      for (int c : children[i]) C[pos++] = (uint8_t)c;
+    }
+  }
   BodyConst* BC = reinterpret_cast<BodyConst*>(M.blob.data() + sizeof(BlobHeader));
   M.rodrigues.assign((size_t)nb * 36, 0.f);
   for (int i = 0; i < nb; ++i) {
@@ -237,6 +323,7 @@ bard_status build_model(const bard_model_desc* d, int device, Model& M) {
     c.type = t; c.parent = M.parent[i]; c.q_off = M.q_off[i]; c.v_off = M.v_off[i];
     c.src = src[i]; c.save = save[i]; c.flags = post_id ? 1 : 0; c.level = M.body_level[i];
     c.anc_lo = (uint32_t)M.anc_mask[i]; c.anc_hi = (uint32_t)(M.anc_mask[i] >> 32);
+    c.child_begin = child_begin[i]; c.child_count = (int32_t)children[i].size();
   }
 
   if (device < 0) return BARD_OK;  // host-only model: tables can be queried, operators refuse to run
