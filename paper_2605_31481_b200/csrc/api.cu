@@ -40,6 +40,7 @@ void bard_model_destroy(bard_model* bm) {
     cudaGetDevice(&prev);
     cudaSetDevice(bm->m.device);
     cudaFree(bm->m.d_blob);
+    if (bm->m.d_jblob) cudaFree(bm->m.d_jblob);
     cudaSetDevice(prev);
   }
   delete bm;
@@ -92,7 +93,8 @@ static bard_status check_call(const char* fn, const bard_model* bm, int64_t B, c
   if (!bm->m.d_blob) { set_error(std::string(fn) + ": host-only model (created with cuda_device < 0)"); return BARD_ERR_INVALID_ARG; }
   if (B < 0) { set_error(std::string(fn) + ": negative batch size"); return BARD_ERR_INVALID_ARG; }
   if (B > 0 && (!a || !b || !c || !d)) { set_error(std::string(fn) + ": NULL device pointer"); return BARD_ERR_INVALID_ARG; }
-  if (B > ((int64_t)1 << 31) - 1024) { set_error(std::string(fn) + ": B too large"); return BARD_ERR_UNSUPPORTED; }
+  // 4 B must fit 32 bits (row-stride arithmetic in the kernels)
+  if (B > ((int64_t)1 << 29)) { set_error(std::string(fn) + ": B too large"); return BARD_ERR_UNSUPPORTED; }
   return BARD_OK;
 }
 

@@ -53,38 +53,63 @@ struct FrameConst {           // 8 words
 // terminated by TASK_END; the inward sweeps of RNEA / CRBA walk the same list backwards.
 enum : uint16_t { TASK_BODY_MASK = 0x00ff, TASK_BAR = 0x0100, TASK_NOOP = 0x0200, TASK_END = 0xffff };
 
-// Header of the device blob; followed by BodyConst[nb], FrameConst[BARD_MAX_FRAMES], then the schedule
-// tables at the byte offsets stored here (each 16-byte aligned).
-struct BlobHeader {           // 32 words
+// Device constants come in three sections, each a multiple of 16 bytes so that it can be staged into shared
+// memory with one TMA bulk copy:
+//   COMMON  BlobHeader | BodyConst[nb] | tasks | children          (all four operators)
+//   M       MHeader | fill lists | rel masks | zero rows           (CRBA only; directly after COMMON)
+//   J       JHeader | FrameConst[16] | columns | zero rows         (Jacobian only; own buffer, rewritten by
+//                                                                   bard_model_set_frames)
+struct BlobHeader {           // 16 words
   int32_t nb, nq, nv, nlevels;
   int32_t nslots;             // number of parent-state slots the outward sweeps need
-  int32_t nframes;
-  int32_t jac_mask_lo, jac_mask_hi;  // union of the frames' ancestor masks
-  float   g[3];               // gravity, world
   int32_t team_warps;         // L
-  int32_t off_tasks;          // uint16 [team_warps][task_stride]
+  int32_t off_tasks;          // uint16 [team_warps][task_stride]   (byte offsets from the start of COMMON)
   int32_t task_stride;
+  float   g[3];               // gravity, world
   int32_t off_children;       // uint8 [nb]: children lists, ascending, concatenated in body order
-  int32_t off_fill;           // uint8 [team_warps][fill_stride]: DOFs (rows of M) each warp fills, 0xff ends
-  int32_t fill_stride;
   int32_t off_dof_body;       // uint8 [nv]
-  int32_t pad[14];
+  int32_t simple;             // 1: every joint is REVOLUTE with T_post = I, or FREE
+  int32_t pad[2];
 };
-static_assert(sizeof(BlobHeader) == 128, "BlobHeader must be 32 words");
+static_assert(sizeof(BlobHeader) == 64, "BlobHeader must be 16 words");
+
+struct MHeader {              // 8 words; byte offsets from the start of the M section
+  int32_t off_fill;           // uint8 [team_warps][fill_stride]: rows of M each warp fills, 0xff ends
+  int32_t fill_stride;
+  int32_t off_rel;            // uint64 [nv]: bit j set <=> j <= i and DOF j sits on an ancestor-or-self body of DOF i
+  int32_t off_zrows;          // uint16 [nzrows]: flat indices i*nv+j of the structurally zero entries (both triangles)
+  int32_t nzrows;             // padded to a multiple of 4 with 0xffff
+  int32_t pad[3];
+};
+struct JHeader {              // 8 words; byte offsets from the start of the J section
+  int32_t nframes;
+  uint32_t jmask_lo, jmask_hi;  // union of the frames' ancestor masks: bodies the Jacobian FK must visit
+  int32_t off_cols;           // uint16 [ncols]: (frame << 8 | dof) of the non-zero columns
+  int32_t ncols;
+  int32_t off_zrows;          // uint16 [nzrows]: flat row indices (f*6+r)*nv+j of the zero rows, padded with 0xffff
+  int32_t nzrows;
+  int32_t pad;
+};
 
 struct Model {
   int device = 0;
   int32_t nb = 0, nq = 0, nv = 0, nlevels = 0, nslots = 0, nframes = 0;
   int32_t team_warps = 1;             // L: warps that share one 32-environment tile (level-parallel schedule)
+  bool simple = false;
   std::vector<int32_t> warp_of;       // body -> warp of its team
   std::vector<int32_t> parent, jtype, level_ptr, level_body, body_level, parent_slot, q_off, v_off, dof_body;
   std::vector<uint64_t> anc_mask;
   std::vector<float> rodrigues;       // nb*36
-  std::vector<unsigned char> blob;    // host copy of the device blob
-  void* d_blob = nullptr;
-  size_t blob_bytes = 0;
+  std::vector<unsigned char> blob;    // host copy of COMMON + M
+  std::vector<unsigned char> jblob;   // host copy of J
+  void* d_blob = nullptr;             // COMMON + M
+  void* d_jblob = nullptr;            // J (allocated for the largest frame set)
+  size_t common_bytes = 0, m_bytes = 0, j_bytes = 0;
   int sm_count = 148;
 };
+
+constexpr size_t kJBlobMax = sizeof(JHeader) + sizeof(FrameConst) * BARD_MAX_FRAMES +
+                             2 * (size_t)BARD_MAX_FRAMES * BARD_MAX_DOF + 2 * 6 * (size_t)BARD_MAX_FRAMES * BARD_MAX_DOF + 64;
 
 void set_error(const std::string& s);
 

@@ -64,6 +64,8 @@ void put(float* dst, const double* src, int n) {
 
 }  // namespace
 
+bard_status set_frames(Model& M, int32_t nframes, const int32_t* body, const double* offset);
+
 bard_status build_model(const bard_model_desc* d, int device, Model& M) {
   if (!d || d->nb < 1 || !d->parent || !d->joint_type || !d->T_pre || !d->mass || !d->com || !d->inertia) {
     set_error("bard_model_create: NULL pointer in description or nb < 1");
@@ -202,53 +204,86 @@ bard_status build_model(const bard_model_desc* d, int device, Model& M) {
   size_t task_stride = 0;
   for (int w = 0; w < L; ++w) task_stride = std::max(task_stride, tasks[w].size() + 1);
   task_stride = (task_stride + 7) & ~(size_t)7;
-  // rows of M (DOFs) each warp fills: longest-processing-time greedy on the row length i + 1
+  // ---- CRBA fill tables.  rel[i]: DOFs j <= i on ancestor-or-self bodies of DOF i (the non-zero part of
+  // row i of the lower triangle).  Rows go to warps by longest-processing-time greedy on popcount(rel).
+  std::vector<uint64_t> rel(M.nv, 0);
+  for (int i = 0; i < M.nv; ++i)
+    for (int j = 0; j <= i; ++j)
+      if ((M.anc_mask[M.dof_body[i]] >> M.dof_body[j]) & 1) rel[i] |= 1ull << j;
   std::vector<std::vector<uint8_t>> fill(L);
   {
+    std::vector<int> order(M.nv);
+    for (int i = 0; i < M.nv; ++i) order[i] = i;
+    auto pc = [&](int i) { return __builtin_popcountll(rel[i]); };
+    std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return pc(x) > pc(y); });
     std::vector<int64_t> work(L, 0);
-    for (int i = M.nv - 1; i >= 0; --i) {
+    for (int i : order) {
       int best = 0;
       for (int w = 1; w < L; ++w)
         if (work[w] < work[best]) best = w;
       fill[best].push_back((uint8_t)i);
-      work[best] += i + 1;
+      work[best] += pc(i) + 2;
     }
   }
   size_t fill_stride = 0;
   for (int w = 0; w < L; ++w) fill_stride = std::max(fill_stride, fill[w].size() + 1);
   fill_stride = (fill_stride + 15) & ~(size_t)15;
+  std::vector<uint16_t> zrows;   // structurally zero entries of M, both triangles
+  for (int i = 0; i < M.nv; ++i)
+    for (int j = 0; j < M.nv; ++j) {
+      const int hi = std::max(i, j), lo = std::min(i, j);
+      if (!((rel[hi] >> lo) & 1)) zrows.push_back((uint16_t)(i * M.nv + j));
+    }
+  while (zrows.size() % 4) zrows.push_back(0xffff);
 
-  // constant blob
+  M.simple = true;
+  for (int i = 0; i < nb; ++i) {
+    const int t = M.jtype[i];
+    const bool post_id = !d->T_post || is_identity12(d->T_post + 12 * i);
+    if (!(t == BARD_JOINT_FREE || (t == BARD_JOINT_REVOLUTE && post_id))) M.simple = false;
+  }
+  if (const char* ev = std::getenv("BARD_FORCE_GENERAL"))   // test knob: run the general kernels on simple models
+    if (std::atoi(ev)) M.simple = false;
+
+  // ---- constant sections COMMON | M
   auto align16 = [](size_t x) { return (x + 15) & ~(size_t)15; };
   const size_t off_bodies = sizeof(BlobHeader);
-  const size_t off_frames = off_bodies + sizeof(BodyConst) * nb;
-  const size_t off_tasks = off_frames + sizeof(FrameConst) * BARD_MAX_FRAMES;
+  const size_t off_tasks = off_bodies + sizeof(BodyConst) * nb;
   const size_t off_children = align16(off_tasks + sizeof(uint16_t) * L * task_stride);
-  const size_t off_fill = align16(off_children + (size_t)nb);
-  const size_t off_dof_body = align16(off_fill + (size_t)L * fill_stride);
-  M.blob_bytes = align16(off_dof_body + (size_t)M.nv);
-  M.blob.assign(M.blob_bytes, 0);
+  const size_t off_dof_body = align16(off_children + (size_t)nb);
+  M.common_bytes = align16(off_dof_body + (size_t)M.nv);
+  const size_t m_off_fill = sizeof(MHeader);
+  const size_t m_off_rel = align16(m_off_fill + (size_t)L * fill_stride);
+  const size_t m_off_zrows = align16(m_off_rel + sizeof(uint64_t) * M.nv);
+  M.m_bytes = align16(m_off_zrows + sizeof(uint16_t) * zrows.size());
+  M.blob.assign(M.common_bytes + M.m_bytes, 0);
   BlobHeader* H = reinterpret_cast<BlobHeader*>(M.blob.data());
-  H->nb = nb; H->nq = M.nq; H->nv = M.nv; H->nlevels = nl; H->nslots = nslots; H->nframes = 0;
+  H->nb = nb; H->nq = M.nq; H->nv = M.nv; H->nlevels = nl; H->nslots = nslots;
   for (int k = 0; k < 3; ++k) H->g[k] = (float)d->gravity[k];
   H->team_warps = L;
   H->off_tasks = (int32_t)off_tasks; H->task_stride = (int32_t)task_stride;
   H->off_children = (int32_t)off_children;
-  H->off_fill = (int32_t)off_fill; H->fill_stride = (int32_t)fill_stride;
   H->off_dof_body = (int32_t)off_dof_body;
+  H->simple = M.simple ? 1 : 0;
   {
     uint16_t* T = reinterpret_cast<uint16_t*>(M.blob.data() + off_tasks);
     for (int w = 0; w < L; ++w) {
       for (size_t k = 0; k < task_stride; ++k) T[w * task_stride + k] = TASK_END;
       for (size_t k = 0; k < tasks[w].size(); ++k) T[w * task_stride + k] = tasks[w][k];
     }
-    uint8_t* F = M.blob.data() + off_fill;
+    uint8_t* D = M.blob.data() + off_dof_body;
+    for (int j = 0; j < M.nv; ++j) D[j] = (uint8_t)M.dof_body[j];
+    unsigned char* MS = M.blob.data() + M.common_bytes;
+    MHeader* MH = reinterpret_cast<MHeader*>(MS);
+    MH->off_fill = (int32_t)m_off_fill; MH->fill_stride = (int32_t)fill_stride;
+    MH->off_rel = (int32_t)m_off_rel; MH->off_zrows = (int32_t)m_off_zrows; MH->nzrows = (int32_t)zrows.size();
+    uint8_t* F = MS + m_off_fill;
     for (int w = 0; w < L; ++w) {
       for (size_t k = 0; k < fill_stride; ++k) F[w * fill_stride + k] = 0xff;
       for (size_t k = 0; k < fill[w].size(); ++k) F[w * fill_stride + k] = fill[w][k];
     }
-    uint8_t* D = M.blob.data() + off_dof_body;
-    for (int j = 0; j < M.nv; ++j) D[j] = (uint8_t)M.dof_body[j];
+    if (M.nv) std::memcpy(MS + m_off_rel, rel.data(), sizeof(uint64_t) * M.nv);
+    if (!zrows.empty()) std::memcpy(MS + m_off_zrows, zrows.data(), sizeof(uint16_t) * zrows.size());
   }
   std::vector<int32_t> child_begin(nb, 0);
   {
@@ -326,10 +361,11 @@ bard_status build_model(const bard_model_desc* d, int device, Model& M) {
     c.child_begin = child_begin[i]; c.child_count = (int32_t)children[i].size();
   }
 
+  set_frames(M, 0, nullptr, nullptr);   // empty J section (host side; the device copy follows below)
   if (device < 0) return BARD_OK;  // host-only model: tables can be queried, operators refuse to run
   int dev_count = 0;
   cudaError_t e = cudaGetDeviceCount(&dev_count);
-  if (e != cudaSuccess || device < 0 || device >= dev_count) {
+  if (e != cudaSuccess || device >= dev_count) {
     set_error(std::string("bard_model_create: no such CUDA device: ") + cudaGetErrorString(e));
     cudaGetLastError();
     return BARD_ERR_CUDA;
@@ -338,42 +374,67 @@ bard_status build_model(const bard_model_desc* d, int device, Model& M) {
   cudaGetDevice(&prev);
   cudaSetDevice(device);
   cudaDeviceGetAttribute(&M.sm_count, cudaDevAttrMultiProcessorCount, device);
-  e = cudaMalloc(&M.d_blob, M.blob_bytes);
-  if (e == cudaSuccess) e = cudaMemcpy(M.d_blob, M.blob.data(), M.blob_bytes, cudaMemcpyHostToDevice);
+  e = cudaMalloc(&M.d_blob, M.blob.size());
+  if (e == cudaSuccess) e = cudaMalloc(&M.d_jblob, kJBlobMax);
+  if (e == cudaSuccess) e = cudaMemcpy(M.d_blob, M.blob.data(), M.blob.size(), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(M.d_jblob, M.jblob.data(), M.jblob.size(), cudaMemcpyHostToDevice);
   cudaSetDevice(prev);
   if (e != cudaSuccess) {
     set_error(std::string("bard_model_create: ") + cudaGetErrorString(e));
     if (M.d_blob) cudaFree(M.d_blob);
-    M.d_blob = nullptr;
+    if (M.d_jblob) cudaFree(M.d_jblob);
+    M.d_blob = M.d_jblob = nullptr;
     return e == cudaErrorMemoryAllocation ? BARD_ERR_ALLOC : BARD_ERR_CUDA;
   }
   return BARD_OK;
 }
 
+// J section: frames, the non-zero columns (frame, dof) and the flat indices of the zero rows of J.
 bard_status set_frames(Model& M, int32_t nframes, const int32_t* body, const double* offset) {
   if (nframes < 0 || (nframes > 0 && !body)) { set_error("bard_model_set_frames: bad arguments"); return BARD_ERR_INVALID_ARG; }
   if (nframes > BARD_MAX_FRAMES) { set_error("bard_model_set_frames: too many frames"); return BARD_ERR_UNSUPPORTED; }
   for (int f = 0; f < nframes; ++f)
     if (body[f] < 0 || body[f] >= M.nb) { set_error("bard_model_set_frames: frame body out of range"); return BARD_ERR_INVALID_ARG; }
-  BlobHeader* H = reinterpret_cast<BlobHeader*>(M.blob.data());
-  FrameConst* F = reinterpret_cast<FrameConst*>(M.blob.data() + sizeof(BlobHeader) + sizeof(BodyConst) * M.nb);
+  auto align16 = [](size_t x) { return (x + 15) & ~(size_t)15; };
+  std::vector<uint16_t> cols, zrows;
   uint64_t uni = 0;
-  std::memset(F, 0, sizeof(FrameConst) * BARD_MAX_FRAMES);
+  for (int f = 0; f < nframes; ++f) {
+    const uint64_t a = M.anc_mask[body[f]];
+    uni |= a;
+    for (int j = 0; j < M.nv; ++j) {
+      if ((a >> M.dof_body[j]) & 1) cols.push_back((uint16_t)((f << 8) | j));
+      else
+        for (int r = 0; r < 6; ++r) zrows.push_back((uint16_t)((f * 6 + r) * M.nv + j));
+    }
+  }
+  while (zrows.size() % 4) zrows.push_back(0xffff);
+  const size_t off_frames = sizeof(JHeader);
+  const size_t off_cols = off_frames + sizeof(FrameConst) * BARD_MAX_FRAMES;
+  const size_t off_zrows = align16(off_cols + sizeof(uint16_t) * cols.size());
+  const size_t bytes = align16(off_zrows + sizeof(uint16_t) * zrows.size());
+  if (bytes > kJBlobMax) { set_error("bard_model_set_frames: internal: J section too large"); return BARD_ERR_UNSUPPORTED; }
+  M.jblob.assign(bytes, 0);
+  JHeader* JH = reinterpret_cast<JHeader*>(M.jblob.data());
+  JH->nframes = nframes;
+  JH->jmask_lo = (uint32_t)uni; JH->jmask_hi = (uint32_t)(uni >> 32);
+  JH->off_cols = (int32_t)off_cols; JH->ncols = (int32_t)cols.size();
+  JH->off_zrows = (int32_t)off_zrows; JH->nzrows = (int32_t)zrows.size();
+  FrameConst* F = reinterpret_cast<FrameConst*>(M.jblob.data() + off_frames);
   for (int f = 0; f < nframes; ++f) {
     F[f].body = body[f];
     for (int k = 0; k < 3; ++k) F[f].off[k] = offset ? (float)offset[3 * f + k] : 0.f;
-    uint64_t a = M.anc_mask[body[f]];
+    const uint64_t a = M.anc_mask[body[f]];
     F[f].anc_lo = (uint32_t)a; F[f].anc_hi = (uint32_t)(a >> 32);
-    uni |= a;
   }
-  H->nframes = nframes;
-  H->jac_mask_lo = (int32_t)(uint32_t)uni; H->jac_mask_hi = (int32_t)(uint32_t)(uni >> 32);
+  if (!cols.empty()) std::memcpy(M.jblob.data() + off_cols, cols.data(), sizeof(uint16_t) * cols.size());
+  if (!zrows.empty()) std::memcpy(M.jblob.data() + off_zrows, zrows.data(), sizeof(uint16_t) * zrows.size());
+  M.j_bytes = bytes;
   M.nframes = nframes;
-  if (!M.d_blob) return BARD_OK;
+  if (!M.d_jblob) return BARD_OK;
   int prev = 0;
   cudaGetDevice(&prev);
   cudaSetDevice(M.device);
-  cudaError_t e = cudaMemcpy(M.d_blob, M.blob.data(), M.blob_bytes, cudaMemcpyHostToDevice);
+  cudaError_t e = cudaMemcpy(M.d_jblob, M.jblob.data(), bytes, cudaMemcpyHostToDevice);
   cudaSetDevice(prev);
   if (e != cudaSuccess) { set_error(std::string("bard_model_set_frames: ") + cudaGetErrorString(e)); return BARD_ERR_CUDA; }
   return BARD_OK;
