@@ -79,7 +79,9 @@ struct MHeader {              // 8 words; byte offsets from the start of the M s
   int32_t off_rel;            // uint64 [nv]: bit j set <=> j <= i and DOF j sits on an ancestor-or-self body of DOF i
   int32_t off_zrows;          // uint16 [nzrows]: flat indices i*nv+j of the structurally zero entries (both triangles)
   int32_t nzrows;             // padded to a multiple of 4 with 0xffff
-  int32_t pad[3];
+  int32_t off_pairs;          // uint8: for row i the DOFs j <= i with M[i][j] != 0 (set bits of rel[i], ascending)
+  int32_t off_pair_ptr;       // uint16 [nv + 1]: row i's pairs are pairs[pair_ptr[i] .. pair_ptr[i+1])
+  int32_t pad;
 };
 struct JHeader {              // 8 words; byte offsets from the start of the J section
   int32_t nframes;
@@ -88,7 +90,7 @@ struct JHeader {              // 8 words; byte offsets from the start of the J s
   int32_t ncols;
   int32_t off_zrows;          // uint16 [nzrows]: flat row indices (f*6+r)*nv+j of the zero rows, padded with 0xffff
   int32_t nzrows;
-  int32_t pad;
+  int32_t off_bframes;        // uint16 [nb]: bit f set <=> frame f is attached to this body
 };
 
 struct Model {
@@ -109,7 +111,8 @@ struct Model {
 };
 
 constexpr size_t kJBlobMax = sizeof(JHeader) + sizeof(FrameConst) * BARD_MAX_FRAMES +
-                             2 * (size_t)BARD_MAX_FRAMES * BARD_MAX_DOF + 2 * 6 * (size_t)BARD_MAX_FRAMES * BARD_MAX_DOF + 64;
+                             2 * (size_t)BARD_MAX_FRAMES * BARD_MAX_DOF + 2 * 6 * (size_t)BARD_MAX_FRAMES * BARD_MAX_DOF +
+                             2 * (size_t)BARD_MAX_BODIES + 96;
 
 void set_error(const std::string& s);
 

@@ -255,7 +255,16 @@ bard_status build_model(const bard_model_desc* d, int device, Model& M) {
   const size_t m_off_fill = sizeof(MHeader);
   const size_t m_off_rel = align16(m_off_fill + (size_t)L * fill_stride);
   const size_t m_off_zrows = align16(m_off_rel + sizeof(uint64_t) * M.nv);
-  M.m_bytes = align16(m_off_zrows + sizeof(uint16_t) * zrows.size());
+  std::vector<uint8_t> pairs;
+  std::vector<uint16_t> pair_ptr(M.nv + 1, 0);
+  for (int i = 0; i < M.nv; ++i) {
+    for (int j = 0; j <= i; ++j)
+      if ((rel[i] >> j) & 1) pairs.push_back((uint8_t)j);
+    pair_ptr[i + 1] = (uint16_t)pairs.size();
+  }
+  const size_t m_off_pairs = align16(m_off_zrows + sizeof(uint16_t) * zrows.size());
+  const size_t m_off_pair_ptr = align16(m_off_pairs + pairs.size());
+  M.m_bytes = align16(m_off_pair_ptr + sizeof(uint16_t) * pair_ptr.size());
   M.blob.assign(M.common_bytes + M.m_bytes, 0);
   BlobHeader* H = reinterpret_cast<BlobHeader*>(M.blob.data());
   H->nb = nb; H->nq = M.nq; H->nv = M.nv; H->nlevels = nl; H->nslots = nslots;
@@ -284,6 +293,9 @@ bard_status build_model(const bard_model_desc* d, int device, Model& M) {
     }
     if (M.nv) std::memcpy(MS + m_off_rel, rel.data(), sizeof(uint64_t) * M.nv);
     if (!zrows.empty()) std::memcpy(MS + m_off_zrows, zrows.data(), sizeof(uint16_t) * zrows.size());
+    MH->off_pairs = (int32_t)m_off_pairs; MH->off_pair_ptr = (int32_t)m_off_pair_ptr;
+    if (!pairs.empty()) std::memcpy(MS + m_off_pairs, pairs.data(), pairs.size());
+    std::memcpy(MS + m_off_pair_ptr, pair_ptr.data(), sizeof(uint16_t) * pair_ptr.size());
   }
   std::vector<int32_t> child_begin(nb, 0);
   {
@@ -411,7 +423,8 @@ bard_status set_frames(Model& M, int32_t nframes, const int32_t* body, const dou
   const size_t off_frames = sizeof(JHeader);
   const size_t off_cols = off_frames + sizeof(FrameConst) * BARD_MAX_FRAMES;
   const size_t off_zrows = align16(off_cols + sizeof(uint16_t) * cols.size());
-  const size_t bytes = align16(off_zrows + sizeof(uint16_t) * zrows.size());
+  const size_t off_bframes = align16(off_zrows + sizeof(uint16_t) * zrows.size());
+  const size_t bytes = align16(off_bframes + sizeof(uint16_t) * M.nb);
   if (bytes > kJBlobMax) { set_error("bard_model_set_frames: internal: J section too large"); return BARD_ERR_UNSUPPORTED; }
   M.jblob.assign(bytes, 0);
   JHeader* JH = reinterpret_cast<JHeader*>(M.jblob.data());
@@ -419,6 +432,11 @@ bard_status set_frames(Model& M, int32_t nframes, const int32_t* body, const dou
   JH->jmask_lo = (uint32_t)uni; JH->jmask_hi = (uint32_t)(uni >> 32);
   JH->off_cols = (int32_t)off_cols; JH->ncols = (int32_t)cols.size();
   JH->off_zrows = (int32_t)off_zrows; JH->nzrows = (int32_t)zrows.size();
+  JH->off_bframes = (int32_t)off_bframes;
+  {
+    uint16_t* BF = reinterpret_cast<uint16_t*>(M.jblob.data() + off_bframes);
+    for (int f = 0; f < nframes; ++f) BF[body[f]] |= (uint16_t)(1u << f);
+  }
   FrameConst* F = reinterpret_cast<FrameConst*>(M.jblob.data() + off_frames);
   for (int f = 0; f < nframes; ++f) {
     F[f].body = body[f];
