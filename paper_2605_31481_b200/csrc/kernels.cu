@@ -809,21 +809,24 @@ int env_int(const char* name, int dflt) {
 }
 bool aligned(const void* p, uintptr_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) == 0; }
 
-// N (environments per lane): 2 when the batch is even, every pointer is 8-byte aligned and there are enough
-// tiles to fill the machine; else 1.  TEAMS per CTA: two tiles share one copy of the constants when the team
+// N (environments per lane): 2 when the batch is even, every pointer is 8-byte aligned, there are enough
+// tiles to fill the machine and the doubled tile state still leaves three CTAs per SM; else 1.  TEAMS per CTA: two tiles share one copy of the constants when the team
 // is narrow; fewer if the state does not fit.  Small CTAs keep the last wave short.
 bool pick_cfg(const Model& m, int64_t B, size_t const_bytes, int team_rows, bool can_pack2, int64_t max_rows,
               LaunchCfg& cfg, std::string& why) {
   const int L = m.team_warps;
-  static const int want_teams = env_int("BARD_TEAMS", 0);      // tuning knobs for experiments
-  static const int want_pack = env_int("BARD_PACK", 0);
-  static const int pack2_min_b = env_int("BARD_PACK2_MIN_B", 32768);
-  int N = (can_pack2 && B >= pack2_min_b) ? 2 : 1;
+  const int want_teams = env_int("BARD_TEAMS", 0);             // tuning / test knobs (read per call)
+  const int want_pack = env_int("BARD_PACK", 0);
+  const int pack2_min_b = env_int("BARD_PACK2_MIN_B", 32768);
+  const size_t fixed = 16 + const_bytes;
+  // two environments per lane halve the non-FP instructions per environment but double the tile's shared
+  // memory: taken only when at least three such CTAs still fit on an SM (measured: DESIGN.md "Tuning")
+  const size_t tile2 = (size_t)team_rows * 64 * sizeof(float);
+  int N = (can_pack2 && B >= pack2_min_b && (fixed + tile2 + 1024) * 3 <= kSmemMax) ? 2 : 1;
   if (want_pack == 1) N = 1;
   if (want_pack == 2 && can_pack2) N = 2;
   int teams = want_teams > 0 ? want_teams : (L <= 4 ? 2 : 1);
   teams = std::max(1, std::min(teams, 8 / L));
-  const size_t fixed = 16 + const_bytes;
   size_t per_team = (size_t)team_rows * 32 * N * sizeof(float);
   if (N == 2 && fixed + per_team > kSmemMax) { N = 1; per_team /= 2; }
   while (teams > 1 && (fixed + per_team * teams) * 2 + 2048 > kSmemMax) --teams;   // keep >= 2 CTAs per SM
@@ -909,9 +912,7 @@ bard_status launch_rnea(const Model& m, int64_t B, const float* q, const float* 
                         void* stream) {
   LaunchCfg cfg;
   std::string why;
-  static const int rnea_pack = env_int("BARD_RNEA_PACK", 0);
-  bool p2 = B % 2 == 0 && aligned(q, 8) && aligned(qd, 8) && aligned(qdd, 8) && aligned(tau, 8);
-  if (rnea_pack == 1) p2 = false;
+  const bool p2 = B % 2 == 0 && aligned(q, 8) && aligned(qd, 8) && aligned(qdd, 8) && aligned(tau, 8);
   if (!pick_cfg(m, B, m.common_bytes, m.nq + 2 * m.nv + 12 * m.nslots + 8 * m.nb, p2, std::max(m.nq, m.nv), cfg, why))
     return refuse("bard_rnea", why);
   auto go = [&](auto kernel, auto id) {

@@ -152,3 +152,53 @@ def test_full_size_sampled(cfg, B):
     assert nerr(M[..., idx], g.o.crba(q64)) <= TOL_DYN
     for a in (pose, J, tau, M):
         assert np.isfinite(a).all()
+
+
+@pytest.mark.parametrize("knobs", [{"BARD_PACK": "2"}, {"BARD_PACK": "1"}, {"BARD_PACK": "2", "BARD_FORCE_GENERAL": "1"},
+                                   {"BARD_TEAM_WARPS": "1"}, {"BARD_TEAM_WARPS": "8", "BARD_PACK": "2"},
+                                   {"BARD_TEAMS": "1"}])
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3])
+def test_every_kernel_instantiation(cfg, knobs, monkeypatch):
+    """The launch heuristics pick (environments per lane, SIMPLE/general kernels, team width) from B and the
+    model; the test knobs force each instantiation on every config, at a size with several tiles and a ragged tail."""
+    for k, v in knobs.items():
+        monkeypatch.setenv(k, v)
+    desc = W.config_robot(cfg)
+    for B in (1000, 130):
+        q, qd, qdd = W.config_states(cfg, B)
+        Gpu(desc).check(q, qd, qdd)
+
+
+def test_odd_batch_and_misaligned_views():
+    """Odd B and output/input pointers that are only 4-byte aligned must take the scalar paths, never fault."""
+    desc = W.config_robot(1)
+    B = 777
+    q, qd, qdd = W.config_states(1, B)
+    g = Gpu(desc)
+    m, dev = g.m, g.dev
+    def off(a):                                    # a tensor whose data pointer is 4 (mod 16)
+        buf = torch.empty(a.size + 1, device=dev)
+        v = buf[1:].view(a.shape)
+        v.copy_(torch.from_numpy(a))
+        return v
+    tq, tqd, tqdd = off(q), off(qd), off(qdd)
+    pose = off(np.full((m.nb, 12, B), np.nan, np.float32)); J = off(np.full((m.nframes, 6, m.nv, B), np.nan, np.float32))
+    tau = off(np.full((m.nv, B), np.nan, np.float32)); M = off(np.full((m.nv, m.nv, B), np.nan, np.float32))
+    s = torch.cuda.current_stream().cuda_stream
+    m.fk(B, tq, pose, s); m.jacobian(B, tq, J, s); m.rnea(B, tq, tqd, tqdd, tau, s); m.crba(B, tq, M, s)
+    torch.cuda.synchronize()
+    q64, qd64, qdd64 = (a.astype(np.float64) for a in (q, qd, qdd))
+    assert nerr(pose.cpu().numpy(), g.o.fk(q64)) <= TOL_KIN
+    assert nerr(J.cpu().numpy(), g.o.jacobian(q64)) <= TOL_KIN
+    assert nerr(tau.cpu().numpy(), g.o.rnea(q64, qd64, qdd64)) <= TOL_DYN
+    assert nerr(M.cpu().numpy(), g.o.crba(q64)) <= TOL_DYN
+
+
+def test_too_many_elements_is_refused_not_wrapped():
+    """Outputs of 2^32 elements or more are refused (32-bit element indices in the kernels)."""
+    desc = W.config_robot(3)
+    m = binding.Model(desc, device=0)
+    t = torch.empty(16, device="cuda:0")
+    with pytest.raises(binding.BardError) as e:
+        m.crba(1 << 23, t, t)                      # 841 * 2^23 > 2^32: refused before any launch
+    assert e.value.code == 3
