@@ -97,6 +97,7 @@ struct Model {
   int device = 0;
   int32_t nb = 0, nq = 0, nv = 0, nlevels = 0, nslots = 0, nframes = 0;
   int32_t team_warps = 1;             // L: warps that share one 32-environment tile (level-parallel schedule)
+  int32_t crba_warps = 1;             // Lc >= L: CRBA adds warps that only join the fill of M
   bool simple = false;
   std::vector<int32_t> warp_of;       // body -> warp of its team
   std::vector<int32_t> parent, jtype, level_ptr, level_body, body_level, parent_slot, q_off, v_off, dof_body;

@@ -785,7 +785,22 @@ __global__ void __launch_bounds__(256) crba_kernel(const void* __restrict__ gcom
     const uint32_t rowo = i * nvu * B + C.e;                 // M[i][.]
     const uint32_t colo = i * B + C.e;                       // M[.][i]
     const int pe_ = pairs_b + ldc_u16(pptr_b + 2 * i + 2);
-    for (int pp = pairs_b + ldc_u16(pptr_b + 2 * i); pp < pe_; ++pp) {
+    int pp = pairs_b + ldc_u16(pptr_b + 2 * i);
+    for (; pp + 1 < pe_; pp += 2) {                          // two pairs per trip: two independent FMA chains
+      const uint32_t j0 = ldc_u8(pp), j1 = ldc_u8(pp + 1);
+      const int s0 = dof + j0 * 6 * RW, s1 = dof + j1 * 6 * RW;
+      const V3<T> a0 = ldrow3<T, RW>(s0), b0 = ldrow3<T, RW>(s0 + 3 * RW);
+      const V3<T> a1 = ldrow3<T, RW>(s1), b1 = ldrow3<T, RW>(s1 + 3 * RW);
+      const T v0_ = dot_acc(b0, Ff, dot(a0, Fn));
+      const T v1_ = dot_acc(b1, Ff, dot(a1, Fn));
+      if (C.valid) {
+        stg(Mout, rowo + j0 * B, v0_);
+        stg(Mout, colo + j0 * nvu * B, v0_);                 // j0 < j1 <= i: never the diagonal
+        stg(Mout, rowo + j1 * B, v1_);
+        if (j1 != i) stg(Mout, colo + j1 * nvu * B, v1_);
+      }
+    }
+    if (pp < pe_) {
       const uint32_t j = ldc_u8(pp);
       const int sj = dof + j * 6 * RW;
       const T val = dot_acc(ldrow3<T, RW>(sj + 3 * RW), Ff, dot(ldrow3<T, RW>(sj), Fn));
@@ -812,9 +827,8 @@ bool aligned(const void* p, uintptr_t a) { return (reinterpret_cast<uintptr_t>(p
 // N (environments per lane): 2 when the batch is even, every pointer is 8-byte aligned, there are enough
 // tiles to fill the machine and the doubled tile state still leaves three CTAs per SM; else 1.  TEAMS per CTA: two tiles share one copy of the constants when the team
 // is narrow; fewer if the state does not fit.  Small CTAs keep the last wave short.
-bool pick_cfg(const Model& m, int64_t B, size_t const_bytes, int team_rows, bool can_pack2, int64_t max_rows,
+bool pick_cfg(int L, int64_t B, size_t const_bytes, int team_rows, bool can_pack2, int64_t max_rows,
               LaunchCfg& cfg, std::string& why) {
-  const int L = m.team_warps;
   const int want_teams = env_int("BARD_TEAMS", 0);             // tuning / test knobs (read per call)
   const int want_pack = env_int("BARD_PACK", 0);
   const int pack2_min_b = env_int("BARD_PACK2_MIN_B", 32768);
@@ -880,7 +894,7 @@ bard_status launch_fk(const Model& m, int64_t B, const float* q, float* pose, vo
   LaunchCfg cfg;
   std::string why;
   const bool p2 = B % 2 == 0 && aligned(q, 8) && aligned(pose, 8);
-  if (!pick_cfg(m, B, m.common_bytes, m.nq + 12 * m.nslots, p2, std::max(12 * m.nb, m.nq), cfg, why)) return refuse("bard_fk", why);
+  if (!pick_cfg(m.team_warps, B, m.common_bytes, m.nq + 12 * m.nslots, p2, std::max(12 * m.nb, m.nq), cfg, why)) return refuse("bard_fk", why);
   auto go = [&](auto kernel, auto id) {
     bard_status s = prep<decltype(id)::value>(kernel, "bard_fk");
     if (s != BARD_OK) return s;
@@ -894,7 +908,7 @@ bard_status launch_jacobian(const Model& m, int64_t B, const float* q, float* J,
   LaunchCfg cfg;
   std::string why;
   const bool p2 = B % 2 == 0 && aligned(q, 8) && aligned(J, 8);
-  if (!pick_cfg(m, B, m.common_bytes + m.j_bytes, m.nq + 12 * m.nslots + 6 * m.nv + 3 * m.nframes, p2,
+  if (!pick_cfg(m.team_warps, B, m.common_bytes + m.j_bytes, m.nq + 12 * m.nslots + 6 * m.nv + 3 * m.nframes, p2,
                 std::max(6 * m.nframes * m.nv, m.nq), cfg, why))
     return refuse("bard_jacobian", why);
   const int vec_ok = (B % 4 == 0) && aligned(J, 16);
@@ -913,7 +927,7 @@ bard_status launch_rnea(const Model& m, int64_t B, const float* q, const float* 
   LaunchCfg cfg;
   std::string why;
   const bool p2 = B % 2 == 0 && aligned(q, 8) && aligned(qd, 8) && aligned(qdd, 8) && aligned(tau, 8);
-  if (!pick_cfg(m, B, m.common_bytes, m.nq + 2 * m.nv + 12 * m.nslots + 8 * m.nb, p2, std::max(m.nq, m.nv), cfg, why))
+  if (!pick_cfg(m.team_warps, B, m.common_bytes, m.nq + 2 * m.nv + 12 * m.nslots + 8 * m.nb, p2, std::max(m.nq, m.nv), cfg, why))
     return refuse("bard_rnea", why);
   auto go = [&](auto kernel, auto id) {
     bard_status s = prep<decltype(id)::value>(kernel, "bard_rnea");
@@ -929,7 +943,7 @@ bard_status launch_crba(const Model& m, int64_t B, const float* q, float* M, voi
   LaunchCfg cfg;
   std::string why;
   const bool p2 = B % 2 == 0 && aligned(q, 8) && aligned(M, 8);
-  if (!pick_cfg(m, B, m.common_bytes + m.m_bytes, m.nq + 12 * m.nslots + 6 * m.nv + 10 * m.nb, p2,
+  if (!pick_cfg(m.crba_warps, B, m.common_bytes + m.m_bytes, m.nq + 12 * m.nslots + 6 * m.nv + 10 * m.nb, p2,
                 std::max(m.nv * m.nv, m.nq), cfg, why))
     return refuse("bard_crba", why);
   const int vec_ok = (B % 4 == 0) && aligned(M, 16);
@@ -937,7 +951,7 @@ bard_status launch_crba(const Model& m, int64_t B, const float* q, float* M, voi
     bard_status s = prep<decltype(id)::value>(kernel, "bard_crba");
     if (s != BARD_OK) return s;
     kernel<<<cfg.grid, cfg.threads, cfg.smem, (cudaStream_t)stream>>>(
-        m.d_blob, (uint32_t)m.common_bytes, (uint32_t)m.m_bytes, m.team_warps, cfg.rcpL, cfg.team_rows, m.nq, m.nv,
+        m.d_blob, (uint32_t)m.common_bytes, (uint32_t)m.m_bytes, m.crba_warps, cfg.rcpL, cfg.team_rows, m.nq, m.nv,
         m.nslots, (uint32_t)B, q, M, vec_ok);
     return finish("bard_crba");
   };

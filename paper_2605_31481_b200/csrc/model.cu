@@ -201,8 +201,19 @@ bard_status build_model(const bard_model_desc* d, int device, Model& M) {
   }
   for (int i = 0; i < nb; ++i) src[i] = M.parent[i] < 0 ? -1 : (reg_fed[i] ? -2 : save[M.parent[i]]);
   M.nslots = nslots;
+  // CRBA runs with Lc >= L warps per team: the extra warps idle through the level sweeps (barrier-only task
+  // lists) and share the fill of M, which parallelises over rows, not over tree levels.
+  int Lc = std::min(8, std::max(L, (M.nv + 3) / 4));
+  if (const char* ev = std::getenv("BARD_CRBA_WARPS")) {   // tuning knob for experiments
+    int v = std::atoi(ev);
+    if (v >= L && v <= 8) Lc = v;
+  }
+  M.crba_warps = Lc;
+  tasks.resize(Lc);
+  for (int w = L; w < Lc; ++w)
+    for (int l = 0; l < nl; ++l) tasks[w].push_back((uint16_t)(TASK_NOOP | TASK_BAR));
   size_t task_stride = 0;
-  for (int w = 0; w < L; ++w) task_stride = std::max(task_stride, tasks[w].size() + 1);
+  for (int w = 0; w < Lc; ++w) task_stride = std::max(task_stride, tasks[w].size() + 1);
   task_stride = (task_stride + 7) & ~(size_t)7;
   // ---- CRBA fill tables.  rel[i]: DOFs j <= i on ancestor-or-self bodies of DOF i (the non-zero part of
   // row i of the lower triangle).  Rows go to warps by longest-processing-time greedy on popcount(rel).
@@ -210,23 +221,23 @@ bard_status build_model(const bard_model_desc* d, int device, Model& M) {
   for (int i = 0; i < M.nv; ++i)
     for (int j = 0; j <= i; ++j)
       if ((M.anc_mask[M.dof_body[i]] >> M.dof_body[j]) & 1) rel[i] |= 1ull << j;
-  std::vector<std::vector<uint8_t>> fill(L);
+  std::vector<std::vector<uint8_t>> fill(Lc);
   {
     std::vector<int> order(M.nv);
     for (int i = 0; i < M.nv; ++i) order[i] = i;
     auto pc = [&](int i) { return __builtin_popcountll(rel[i]); };
     std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return pc(x) > pc(y); });
-    std::vector<int64_t> work(L, 0);
+    std::vector<int64_t> work(Lc, 0);
     for (int i : order) {
       int best = 0;
-      for (int w = 1; w < L; ++w)
+      for (int w = 1; w < Lc; ++w)
         if (work[w] < work[best]) best = w;
       fill[best].push_back((uint8_t)i);
       work[best] += pc(i) + 2;
     }
   }
   size_t fill_stride = 0;
-  for (int w = 0; w < L; ++w) fill_stride = std::max(fill_stride, fill[w].size() + 1);
+  for (int w = 0; w < Lc; ++w) fill_stride = std::max(fill_stride, fill[w].size() + 1);
   fill_stride = (fill_stride + 15) & ~(size_t)15;
   std::vector<uint16_t> zrows;   // structurally zero entries of M, both triangles
   for (int i = 0; i < M.nv; ++i)
@@ -249,11 +260,11 @@ bard_status build_model(const bard_model_desc* d, int device, Model& M) {
   auto align16 = [](size_t x) { return (x + 15) & ~(size_t)15; };
   const size_t off_bodies = sizeof(BlobHeader);
   const size_t off_tasks = off_bodies + sizeof(BodyConst) * nb;
-  const size_t off_children = align16(off_tasks + sizeof(uint16_t) * L * task_stride);
+  const size_t off_children = align16(off_tasks + sizeof(uint16_t) * Lc * task_stride);
   const size_t off_dof_body = align16(off_children + (size_t)nb);
   M.common_bytes = align16(off_dof_body + (size_t)M.nv);
   const size_t m_off_fill = sizeof(MHeader);
-  const size_t m_off_rel = align16(m_off_fill + (size_t)L * fill_stride);
+  const size_t m_off_rel = align16(m_off_fill + (size_t)Lc * fill_stride);
   const size_t m_off_zrows = align16(m_off_rel + sizeof(uint64_t) * M.nv);
   std::vector<uint8_t> pairs;
   std::vector<uint16_t> pair_ptr(M.nv + 1, 0);
@@ -276,7 +287,7 @@ bard_status build_model(const bard_model_desc* d, int device, Model& M) {
   H->simple = M.simple ? 1 : 0;
   {
     uint16_t* T = reinterpret_cast<uint16_t*>(M.blob.data() + off_tasks);
-    for (int w = 0; w < L; ++w) {
+    for (int w = 0; w < Lc; ++w) {
       for (size_t k = 0; k < task_stride; ++k) T[w * task_stride + k] = TASK_END;
       for (size_t k = 0; k < tasks[w].size(); ++k) T[w * task_stride + k] = tasks[w][k];
     }
@@ -287,7 +298,7 @@ bard_status build_model(const bard_model_desc* d, int device, Model& M) {
     MH->off_fill = (int32_t)m_off_fill; MH->fill_stride = (int32_t)fill_stride;
     MH->off_rel = (int32_t)m_off_rel; MH->off_zrows = (int32_t)m_off_zrows; MH->nzrows = (int32_t)zrows.size();
     uint8_t* F = MS + m_off_fill;
-    for (int w = 0; w < L; ++w) {
+    for (int w = 0; w < Lc; ++w) {
       for (size_t k = 0; k < fill_stride; ++k) F[w * fill_stride + k] = 0xff;
       for (size_t k = 0; k < fill[w].size(); ++k) F[w * fill_stride + k] = fill[w][k];
     }
