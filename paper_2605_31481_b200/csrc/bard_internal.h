@@ -31,7 +31,7 @@ struct BodyConst {
   int32_t src;                // 56  where the parent's state is: -1 world, -2 registers of the same warp
                               //     (the task this warp processed just before), >=0 shared-memory slot
   int32_t save;               // 57  slot this body's state is saved to for children on other warps (-1: none)
-  int32_t flags;              // 58  bit0: T_post is identity (a = b = 0, Sl = 0)
+  int32_t flags;              // 58  bit0: T_post is identity (a = b = 0, Sl = 0); bits 8..15: index among free-joint bodies
   int32_t level;              // 59
   uint32_t anc_lo, anc_hi;    // 60, 61  ancestor-or-self mask of this body
   int32_t child_begin;        // 62  first entry of this body's children in the CHILDREN table
@@ -73,15 +73,18 @@ struct BlobHeader {           // 16 words
 };
 static_assert(sizeof(BlobHeader) == 64, "BlobHeader must be 16 words");
 
-struct MHeader {              // 8 words; byte offsets from the start of the M section
+struct MHeader {              // 12 words; byte offsets from the start of the M section
   int32_t off_fill;           // uint8 [team_warps][fill_stride]: rows of M each warp fills, 0xff ends
   int32_t fill_stride;
   int32_t off_rel;            // uint64 [nv]: bit j set <=> j <= i and DOF j sits on an ancestor-or-self body of DOF i
   int32_t off_zrows;          // uint16 [nzrows]: flat indices i*nv+j of the structurally zero entries (both triangles)
   int32_t nzrows;             // padded to a multiple of 4 with 0xffff
-  int32_t off_pairs;          // uint8: for row i the DOFs j <= i with M[i][j] != 0 (set bits of rel[i], ascending)
+  int32_t off_pairs;          // uint8: for row i the DOFs j <= i with M[i][j] != 0, EXCEPT the DOFs of free-joint
+                              //        bodies that are proper ancestors of row i's body (those go through fanc)
   int32_t off_pair_ptr;       // uint16 [nv + 1]: row i's pairs are pairs[pair_ptr[i] .. pair_ptr[i+1])
-  int32_t pad;
+  int32_t off_fanc;           // uint8: for row i the free-joint bodies that are proper ancestors of its body
+  int32_t off_fanc_ptr;       // uint16 [nv + 1]
+  int32_t pad[3];
 };
 struct JHeader {              // 8 words; byte offsets from the start of the J section
   int32_t nframes;
@@ -95,7 +98,7 @@ struct JHeader {              // 8 words; byte offsets from the start of the J s
 
 struct Model {
   int device = 0;
-  int32_t nb = 0, nq = 0, nv = 0, nlevels = 0, nslots = 0, nframes = 0;
+  int32_t nb = 0, nq = 0, nv = 0, nlevels = 0, nslots = 0, nframes = 0, nfree = 0;
   int32_t team_warps = 1;             // L: warps that share one 32-environment tile (level-parallel schedule)
   int32_t crba_warps = 1;             // Lc >= L: CRBA adds warps that only join the fill of M
   bool simple = false;

@@ -688,11 +688,13 @@ __global__ void __launch_bounds__(256) rnea_kernel(const void* __restrict__ gcom
 // (m, h, I: 10 floats), so the backward sweep  I^c_parent += X^T I^c_child X degenerates to
 // ten additions (X = identity between world-frame quantities), and M_ij = s_j . (I^c_i s_i) for every
 // ancestor DOF j needs no transform along the walk.  The screws s are the eq. (7) columns (store_screws).
-// team rows: q[nq] | pose slots[12 nslots] | screws[6 nv] | inertia[10 nb]
+// team rows: q[nq] | pose slots[12 nslots] | screws[6 nv] | inertia[10 nb] | poses of free-joint bodies[12 nfree]
 // Phase 1 (outward, level-parallel): FK, screws, world-frame body inertias.
 // Phase 2 (inward, level-parallel): a body adds its children's composites in ascending child order.
 // Phase 3: the rows of M are dealt to the team's warps (host LPT schedule); the warp that owns row i walks
-//          the host-built list of DOFs j <= i on ancestor bodies and writes M[i][j] and M[j][i].
+//          the host-built list of DOFs j <= i on ancestor bodies and writes M[i][j] and M[j][i]; the six
+//          entries against a free-joint ancestor (floating base) come from ONE force transform into that
+//          body's frame, [R^T f ; R^T (n + f x p)], instead of six 6-term dot products.
 // Phase 4: the structurally zero entries.  Every element of M is written exactly once.
 template <bool SIMPLE, int N>
 __global__ void __launch_bounds__(256) crba_kernel(const void* __restrict__ gcommon, uint32_t cbytes, uint32_t mbytes, int L,
@@ -708,6 +710,7 @@ __global__ void __launch_bounds__(256) crba_kernel(const void* __restrict__ gcom
   const int slots = C.st + nq * RW;
   const int dof = slots + nslots * 12 * RW;                    // 6 rows per DOF
   const int ic = dof + nv * 6 * RW;                            // 10 rows per body: m h(3) I(6)
+  const int fpose = ic + ldci(C.common + H_NB) * 10 * RW;      // 12 rows per free-joint body: R p
   Pose<T> cur;
   int ntask = 0;
   for (int k = 0;; ++k) {
@@ -720,6 +723,12 @@ __global__ void __launch_bounds__(256) crba_kernel(const void* __restrict__ gcom
       T u, w;
       fk_body<SIMPLE, T, RW>(body, m, qs, slots, cur, u, w);
       store_screws<SIMPLE, T, RW>(body, m, cur, dof);
+      if (m.type == BARD_JOINT_FREE) {
+        const int fp = fpose + ((m.flags >> 8) & 0xff) * 12 * RW;
+#pragma unroll
+        for (int j = 0; j < 9; ++j) sts(fp + j * RW, cur.R.m[j]);
+        strow3<RW>(fp + 9 * RW, cur.p);
+      }
       // body inertia about the world origin: h' = R h + m p ; with h'' = R h + m p / 2:
       // I' = R Io R^T + 2 (p . h'') 1 - (h'' p^T + p h''^T)
       const Inertia in = load_inertia(body);
@@ -769,6 +778,8 @@ __global__ void __launch_bounds__(256) crba_kernel(const void* __restrict__ gcom
   const int rows_b = xb + ldci(C.extra + 0) + C.w * ldci(C.extra + 1);
   const int pairs_b = xb + ldci(C.extra + 5);
   const int pptr_b = xb + ldci(C.extra + 6);
+  const int fanc_b = xb + ldci(C.extra + 7);
+  const int fptr_b = xb + ldci(C.extra + 8);
   const uint32_t nvu = nv;
   for (int k = 0;; ++k) {
     const uint32_t i = ldc_u8(rows_b + k);
@@ -807,6 +818,26 @@ __global__ void __launch_bounds__(256) crba_kernel(const void* __restrict__ gcom
       if (C.valid) {
         stg(Mout, rowo + j * B, val);
         if (j != i) stg(Mout, colo + j * nvu * B, val);
+      }
+    }
+    // free-joint ancestors: M[i][v .. v+5] = [R^T Ff ; R^T (Fn + Ff x p)]  (linear block, angular block)
+    const int fe_ = fanc_b + ldc_u16(fptr_b + 2 * i + 2);
+    for (int fq = fanc_b + ldc_u16(fptr_b + 2 * i); fq < fe_; ++fq) {
+      const int fbody = C.bodies + 64 * (int)ldc_u8(fq);
+      const uint32_t vo = (uint32_t)ldci(fbody + 55);
+      const int fp = fpose + ((ldci(fbody + 58) >> 8) & 0xff) * 12 * RW;
+      M3<T> R;
+#pragma unroll
+      for (int j = 0; j < 9; ++j) R.m[j] = lds<T>(fp + j * RW);
+      const V3<T> p = ldrow3<T, RW>(fp + 9 * RW);
+      const V3<T> fl = mulT(R, Ff);
+      const V3<T> nn = mulT(R, cross_acc(Ff, p, Fn));
+      if (C.valid) {
+        const uint32_t ro = rowo + vo * B, co = colo + vo * nvu * B, cs = nvu * B;
+        stg(Mout, ro, fl.x); stg(Mout, ro + B, fl.y); stg(Mout, ro + 2 * B, fl.z);
+        stg(Mout, ro + 3 * B, nn.x); stg(Mout, ro + 4 * B, nn.y); stg(Mout, ro + 5 * B, nn.z);
+        stg(Mout, co, fl.x); stg(Mout, co + cs, fl.y); stg(Mout, co + 2 * cs, fl.z);
+        stg(Mout, co + 3 * cs, nn.x); stg(Mout, co + 4 * cs, nn.y); stg(Mout, co + 5 * cs, nn.z);
       }
     }
   }
@@ -943,7 +974,7 @@ bard_status launch_crba(const Model& m, int64_t B, const float* q, float* M, voi
   LaunchCfg cfg;
   std::string why;
   const bool p2 = B % 2 == 0 && aligned(q, 8) && aligned(M, 8);
-  if (!pick_cfg(m.crba_warps, B, m.common_bytes + m.m_bytes, m.nq + 12 * m.nslots + 6 * m.nv + 10 * m.nb, p2,
+  if (!pick_cfg(m.crba_warps, B, m.common_bytes + m.m_bytes, m.nq + 12 * m.nslots + 6 * m.nv + 10 * m.nb + 12 * m.nfree, p2,
                 std::max(m.nv * m.nv, m.nq), cfg, why))
     return refuse("bard_crba", why);
   const int vec_ok = (B % 4 == 0) && aligned(M, 16);

@@ -266,16 +266,24 @@ bard_status build_model(const bard_model_desc* d, int device, Model& M) {
   const size_t m_off_fill = sizeof(MHeader);
   const size_t m_off_rel = align16(m_off_fill + (size_t)Lc * fill_stride);
   const size_t m_off_zrows = align16(m_off_rel + sizeof(uint64_t) * M.nv);
-  std::vector<uint8_t> pairs;
-  std::vector<uint16_t> pair_ptr(M.nv + 1, 0);
+  std::vector<uint8_t> pairs, fanc;
+  std::vector<uint16_t> pair_ptr(M.nv + 1, 0), fanc_ptr(M.nv + 1, 0);
   for (int i = 0; i < M.nv; ++i) {
-    for (int j = 0; j <= i; ++j)
-      if ((rel[i] >> j) & 1) pairs.push_back((uint8_t)j);
+    const int bi = M.dof_body[i];
+    for (int j = 0; j <= i; ++j) {
+      const int bj = M.dof_body[j];
+      if (((rel[i] >> j) & 1) && !(M.jtype[bj] == BARD_JOINT_FREE && bj != bi)) pairs.push_back((uint8_t)j);
+    }
     pair_ptr[i + 1] = (uint16_t)pairs.size();
+    for (int b = 0; b < bi; ++b)
+      if (M.jtype[b] == BARD_JOINT_FREE && ((M.anc_mask[bi] >> b) & 1)) fanc.push_back((uint8_t)b);
+    fanc_ptr[i + 1] = (uint16_t)fanc.size();
   }
   const size_t m_off_pairs = align16(m_off_zrows + sizeof(uint16_t) * zrows.size());
   const size_t m_off_pair_ptr = align16(m_off_pairs + pairs.size());
-  M.m_bytes = align16(m_off_pair_ptr + sizeof(uint16_t) * pair_ptr.size());
+  const size_t m_off_fanc = align16(m_off_pair_ptr + sizeof(uint16_t) * pair_ptr.size());
+  const size_t m_off_fanc_ptr = align16(m_off_fanc + fanc.size());
+  M.m_bytes = align16(m_off_fanc_ptr + sizeof(uint16_t) * fanc_ptr.size());
   M.blob.assign(M.common_bytes + M.m_bytes, 0);
   BlobHeader* H = reinterpret_cast<BlobHeader*>(M.blob.data());
   H->nb = nb; H->nq = M.nq; H->nv = M.nv; H->nlevels = nl; H->nslots = nslots;
@@ -307,6 +315,9 @@ bard_status build_model(const bard_model_desc* d, int device, Model& M) {
     MH->off_pairs = (int32_t)m_off_pairs; MH->off_pair_ptr = (int32_t)m_off_pair_ptr;
     if (!pairs.empty()) std::memcpy(MS + m_off_pairs, pairs.data(), pairs.size());
     std::memcpy(MS + m_off_pair_ptr, pair_ptr.data(), sizeof(uint16_t) * pair_ptr.size());
+    MH->off_fanc = (int32_t)m_off_fanc; MH->off_fanc_ptr = (int32_t)m_off_fanc_ptr;
+    if (!fanc.empty()) std::memcpy(MS + m_off_fanc, fanc.data(), fanc.size());
+    std::memcpy(MS + m_off_fanc_ptr, fanc_ptr.data(), sizeof(uint16_t) * fanc_ptr.size());
   }
   std::vector<int32_t> child_begin(nb, 0);
   {
@@ -380,6 +391,7 @@ bard_status build_model(const bard_model_desc* d, int device, Model& M) {
     put(c.Io, Io, 6);
     c.type = t; c.parent = M.parent[i]; c.q_off = M.q_off[i]; c.v_off = M.v_off[i];
     c.src = src[i]; c.save = save[i]; c.flags = post_id ? 1 : 0; c.level = M.body_level[i];
+    if (t == BARD_JOINT_FREE) c.flags |= (M.nfree++) << 8;
     c.anc_lo = (uint32_t)M.anc_mask[i]; c.anc_hi = (uint32_t)(M.anc_mask[i] >> 32);
     c.child_begin = child_begin[i]; c.child_count = (int32_t)children[i].size();
   }
