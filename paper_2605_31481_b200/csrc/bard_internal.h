@@ -103,6 +103,7 @@ struct Model {
   int32_t crba_warps = 1;             // Lc >= L: CRBA adds warps that only join the fill of M
   bool simple = false;
   std::vector<int32_t> warp_of;       // body -> warp of its team
+  std::vector<int32_t> free_index;    // body -> index among free-joint bodies (-1 otherwise)
   std::vector<int32_t> parent, jtype, level_ptr, level_body, body_level, parent_slot, q_off, v_off, dof_body;
   std::vector<uint64_t> anc_mask;
   std::vector<float> rodrigues;       // nb*36

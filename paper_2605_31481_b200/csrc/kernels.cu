@@ -232,11 +232,16 @@ __device__ __forceinline__ void team_sync(const Ctx& c) {
   if (c.L > 1) asm volatile("bar.sync %0, %1;" ::"r"(c.bar_id), "r"(c.bar_cnt) : "memory");
 }
 
+// Where each staged input row lands among the team's state rows (RNEA parks q / qd / qdd of a body in the rows
+// that later hold that body's force and joint scalars, so the inputs cost no shared memory of their own).
+struct RowMap { uint16_t q[128], qd[64], qdd[64]; };
+
 // `rcpL` = ceil(65536 / L): warp / L as a multiply and a shift (exact for warp < 64).
+// map == nullptr: input row r of array k lands in state row (rows of the arrays before it) + r.
 template <int N>
 __device__ __forceinline__ Ctx setup(const void* gcommon, uint32_t cbytes, const void* gextra, uint32_t xbytes, int L,
                                      uint32_t rcpL, int team_rows, uint32_t B, const float* in0, int n0, const float* in1,
-                                     int n1, const float* in2, int n2) {
+                                     int n1, const float* in2, int n2, const RowMap* map = nullptr) {
   constexpr int RW = 32 * N;
   const uint32_t bar_a = smem_u32(smf);
   Ctx c;
@@ -263,9 +268,15 @@ __device__ __forceinline__ Ctx setup(const void* gcommon, uint32_t cbytes, const
   }
   // stage the team's input rows; warp w takes rows w, w + L, ...
   const uint32_t st_a = bar_a + 4u * c.st;
-  for (int r = c.w; r < n0; r += L) cp_async_row<N>(st_a + 4u * (r * RW), in0 + ((uint32_t)r * B + el));
-  for (int r = c.w; r < n1; r += L) cp_async_row<N>(st_a + 4u * ((n0 + r) * RW), in1 + ((uint32_t)r * B + el));
-  for (int r = c.w; r < n2; r += L) cp_async_row<N>(st_a + 4u * ((n0 + n1 + r) * RW), in2 + ((uint32_t)r * B + el));
+  if (map) {
+    for (int r = c.w; r < n0; r += L) cp_async_row<N>(st_a + 4u * (map->q[r] * RW), in0 + ((uint32_t)r * B + el));
+    for (int r = c.w; r < n1; r += L) cp_async_row<N>(st_a + 4u * (map->qd[r] * RW), in1 + ((uint32_t)r * B + el));
+    for (int r = c.w; r < n2; r += L) cp_async_row<N>(st_a + 4u * (map->qdd[r] * RW), in2 + ((uint32_t)r * B + el));
+  } else {
+    for (int r = c.w; r < n0; r += L) cp_async_row<N>(st_a + 4u * (r * RW), in0 + ((uint32_t)r * B + el));
+    for (int r = c.w; r < n1; r += L) cp_async_row<N>(st_a + 4u * ((n0 + r) * RW), in1 + ((uint32_t)r * B + el));
+    for (int r = c.w; r < n2; r += L) cp_async_row<N>(st_a + 4u * ((n0 + n1 + r) * RW), in2 + ((uint32_t)r * B + el));
+  }
   cp_async_wait_all();
   __syncthreads();          // mbarrier init visible to all; staged rows visible to the other warps
   mbar_wait(bar_a);
@@ -329,21 +340,21 @@ __device__ __forceinline__ void free_Rt(int body, int qrow, M3<T>& R, V3<T>& t) 
   R = mul(R0, Rq);
   t = mul_acc(R0, p, t0);
 }
-// Local transform of a body from the team's staged q rows (qs = float index of q row 0 for this lane).
+// Local transform of a body from its staged q row(s) (qrow = float index of the body's first q row for this lane).
 // Returns true when the translation is the per-environment tv, false when it is the constant tc.
 template <bool SIMPLE, class T, int RW>
-__device__ __forceinline__ bool local_Rt(int body, const Meta& m, int qs, M3<T>& R, V3<float>& tc, V3<T>& tv, T& u, T& w) {
+__device__ __forceinline__ bool local_Rt(int body, const Meta& m, int qrow, M3<T>& R, V3<float>& tc, V3<T>& tv, T& u, T& w) {
   if (m.type == BARD_JOINT_FREE) {
     u = 0.f; w = 0.f;
-    free_Rt<T, RW>(body, qs + m.q_off * RW, R, tv);
+    free_Rt<T, RW>(body, qrow, R, tv);
     return true;
   }
   if (SIMPLE || m.type == BARD_JOINT_REVOLUTE) {
     T s, co;
-    sincos_fast(lds<T>(qs + m.q_off * RW), s, co);
+    sincos_fast(lds<T>(qrow), s, co);
     u = s; w = T(1.0f) - co;
   } else if (m.type == BARD_JOINT_PRISMATIC) {
-    u = lds<T>(qs + m.q_off * RW); w = 0.f;
+    u = lds<T>(qrow); w = 0.f;
   } else {
     u = 0.f; w = 0.f;
   }
@@ -387,7 +398,7 @@ __device__ __forceinline__ void save_pose(int save, const Pose<T>& P, int slots)
 template <bool SIMPLE, class T, int RW>
 __device__ __forceinline__ void fk_body(int body, const Meta& m, int qs, int slots, Pose<T>& cur, T& u, T& w) {
   M3<T> R; V3<float> tc; V3<T> tv;
-  const bool var_t = local_Rt<SIMPLE, T, RW>(body, m, qs, R, tc, tv, u, w);
+  const bool var_t = local_Rt<SIMPLE, T, RW>(body, m, qs + m.q_off * RW, R, tc, tv, u, w);
   fetch_parent<T, RW>(m.src, cur, slots);
   if (var_t) compose(m.src, cur, R, tv);
   else compose(m.src, cur, R, tc);
@@ -543,7 +554,10 @@ __global__ void __launch_bounds__(256) jacobian_kernel(const void* __restrict__ 
 
 // ============================================================================= RNEA kernel (a4 + a5)
 // Body-frame recursion, internal order [angular; linear].
-// team rows: q[nq] | qd[nv] | qdd[nv] | motion slots[12 nslots] (v.w v.v a.w a.v) | force[6 nb] (n f) | uw[2 nb]
+// team rows: motion slots[12 nslots] (v.w v.v a.w a.v) | body regions[8 nb] (n(3) f(3) u w) | free-joint inputs[19 nfree]
+// The staged inputs of a 1-DOF body are parked in its own region until its outward task has read them
+// (qd -> row 0, qdd -> row 1, q -> row 6); a free joint's q(7) qd(6) qdd(6) get 19 rows of their own (q is
+// read again by the inward pass).
 // Outward (level-parallel, eq. (6)): v, a of the parent come from the registers of this warp's
 // previous task, a shared-memory slot, or the world (v = 0, a = -g: gravity trick); the net body force f_i and
 // the joint scalars (u, w) are parked in shared memory.
@@ -576,17 +590,15 @@ template <bool SIMPLE, int N>
 __global__ void __launch_bounds__(256) rnea_kernel(const void* __restrict__ gcommon, uint32_t cbytes, int L, uint32_t rcpL,
                                                    int team_rows, int nq, int nv, int nb, int nslots, uint32_t B,
                                                    const float* __restrict__ q, const float* __restrict__ qd,
-                                                   const float* __restrict__ qdd, float* __restrict__ tau) {
+                                                   const float* __restrict__ qdd, float* __restrict__ tau,
+                                                   const __grid_constant__ RowMap map) {
   using T = typename Pack<N>::T;
   constexpr int RW = 32 * N;
-  const Ctx C = setup<N>(gcommon, cbytes, nullptr, 0, L, rcpL, team_rows, B, q, nq, qd, nv, qdd, nv);
+  const Ctx C = setup<N>(gcommon, cbytes, nullptr, 0, L, rcpL, team_rows, B, q, nq, qd, nv, qdd, nv, &map);
   const int children_b = 16 + ldci(C.common + H_OFF_CHILDREN);
-  const int qs = C.st;
-  const int qds = qs + nq * RW;
-  const int qdds = qds + nv * RW;
-  const int slots = C.st + (nq + 2 * nv) * RW;
-  const int bst = slots + nslots * 12 * RW;
-  const int uw = bst + nb * 6 * RW;
+  const int slots = C.st;
+  const int bst = slots + nslots * 12 * RW;                    // 8 rows per body
+  const int fin = bst + nb * 8 * RW;                           // 19 rows per free-joint body
   const V3<float> ng = {-ldc(C.common + H_G), -ldc(C.common + H_G + 1), -ldc(C.common + H_G + 2)};
   Motion<T> cur;                                               // this warp's previous body: v and a
   int ntask = 0;
@@ -599,18 +611,20 @@ __global__ void __launch_bounds__(256) rnea_kernel(const void* __restrict__ gcom
       const Meta m = load_meta(body);
       const Inertia in = load_inertia(body);
       M3<T> R; V3<float> tc; V3<T> tv; T u, w;
-      const bool var_t = local_Rt<SIMPLE, T, RW>(body, m, qs, R, tc, tv, u, w);
-      // joint velocity / acceleration in the body frame: S qd, S qdd
       const bool is_free = m.type == BARD_JOINT_FREE;
+      const int b = bst + i * 8 * RW;
+      const int fi = fin + ((m.flags >> 8) & 0xff) * 19 * RW;
+      const bool var_t = local_Rt<SIMPLE, T, RW>(body, m, is_free ? fi : b + 6 * RW, R, tc, tv, u, w);
+      // joint velocity / acceleration in the body frame: S qd, S qdd
       const bool haslin = is_free || !SIMPLE;
       const V3<T> zero = {T(0.f), T(0.f), T(0.f)};
       V3<T> vJw = zero, vJv = zero, aJw = zero, aJv = zero;
       if (is_free) {
-        const int d1 = qds + m.v_off * RW, d2 = qdds + m.v_off * RW;
+        const int d1 = fi + 7 * RW, d2 = fi + 13 * RW;
         vJw = ldrow3<T, RW>(d1 + 3 * RW); vJv = ldrow3<T, RW>(d1);
         aJw = ldrow3<T, RW>(d2 + 3 * RW); aJv = ldrow3<T, RW>(d2);
       } else if (SIMPLE || m.type != BARD_JOINT_FIXED) {
-        const T qd_i = lds<T>(qds + m.v_off * RW), qdd_i = lds<T>(qdds + m.v_off * RW);
+        const T qd_i = lds<T>(b), qdd_i = lds<T>(b + RW);
         vJw = scale(qd_i, in.Sw); aJw = scale(qdd_i, in.Sw);
         if (!SIMPLE) { vJv = scale(qd_i, in.Sl); aJv = scale(qdd_i, in.Sl); }
       }
@@ -634,9 +648,8 @@ __global__ void __launch_bounds__(256) rnea_kernel(const void* __restrict__ gcom
       const V3<T> f2_ = cross_acc(cur.aw, in.h, scale(in.mass, cur.av));
       const V3<T> n = cross_acc(cur.vv, f1, cross_acc(cur.vw, n1, n2));
       const V3<T> f = cross_acc(cur.vw, f1, f2_);
-      const int b = bst + i * 6 * RW;
       strow3<RW>(b, n); strow3<RW>(b + 3 * RW, f);
-      sts(uw + (2 * i) * RW, u); sts(uw + (2 * i + 1) * RW, w);
+      sts(b + 6 * RW, u); sts(b + 7 * RW, w);
       if (m.save >= 0) {
         const int s = slots + m.save * 12 * RW;
         strow3<RW>(s, cur.vw); strow3<RW>(s + 3 * RW, cur.vv); strow3<RW>(s + 6 * RW, cur.aw); strow3<RW>(s + 9 * RW, cur.av);
@@ -652,10 +665,10 @@ __global__ void __launch_bounds__(256) rnea_kernel(const void* __restrict__ gcom
     const int i = tk & TASK_BODY_MASK;
     const int body = C.bodies + 64 * i;
     const Meta m = load_meta(body);
-    const int b = bst + i * 6 * RW;
+    const int b = bst + i * 8 * RW;
     V3<T> n = ldrow3<T, RW>(b), f = ldrow3<T, RW>(b + 3 * RW);
     for (int cc = 0; cc < m.child_count; ++cc) {
-      const int cb = bst + (int)ldc_u8(children_b + m.child_begin + cc) * 6 * RW;
+      const int cb = bst + (int)ldc_u8(children_b + m.child_begin + cc) * 8 * RW;
       n = n + ldrow3<T, RW>(cb); f = f + ldrow3<T, RW>(cb + 3 * RW);
     }
     if (C.valid) {
@@ -673,8 +686,8 @@ __global__ void __launch_bounds__(256) rnea_kernel(const void* __restrict__ gcom
     if (m.parent >= 0) {
       M3<T> R; V3<float> tc; V3<T> tv;
       bool var_t = true;
-      if (m.type == BARD_JOINT_FREE) free_Rt<T, RW>(body, qs + m.q_off * RW, R, tv);
-      else { joint_Rt<SIMPLE, T>(body, m.flags, lds<T>(uw + (2 * i) * RW), lds<T>(uw + (2 * i + 1) * RW), R, tc, tv); var_t = !SIMPLE; }
+      if (m.type == BARD_JOINT_FREE) free_Rt<T, RW>(body, fin + ((m.flags >> 8) & 0xff) * 19 * RW, R, tv);
+      else { joint_Rt<SIMPLE, T>(body, m.flags, lds<T>(b + 6 * RW), lds<T>(b + 7 * RW), R, tc, tv); var_t = !SIMPLE; }
       const V3<T> fp = mul(R, f);
       if (var_t) strow3<RW>(b, cross_acc(tv, fp, mul(R, n)));
       else strow3<RW>(b, cross_acc(tc, fp, mul(R, n)));
@@ -958,14 +971,25 @@ bard_status launch_rnea(const Model& m, int64_t B, const float* q, const float* 
   LaunchCfg cfg;
   std::string why;
   const bool p2 = B % 2 == 0 && aligned(q, 8) && aligned(qd, 8) && aligned(qdd, 8) && aligned(tau, 8);
-  if (!pick_cfg(m.team_warps, B, m.common_bytes, m.nq + 2 * m.nv + 12 * m.nslots + 8 * m.nb, p2, std::max(m.nq, m.nv), cfg, why))
+  if (!pick_cfg(m.team_warps, B, m.common_bytes, 12 * m.nslots + 8 * m.nb + 19 * m.nfree, p2, std::max(m.nq, m.nv), cfg, why))
     return refuse("bard_rnea", why);
+  RowMap map;                                                  // where the staged input rows land (see rnea_kernel)
+  for (int i = 0; i < m.nb; ++i) {
+    const int reg = 12 * m.nslots + 8 * i, qo = m.q_off[i], vo = m.v_off[i];
+    if (m.jtype[i] == BARD_JOINT_FREE) {
+      const int fi = 12 * m.nslots + 8 * m.nb + 19 * m.free_index[i];
+      for (int k = 0; k < 7; ++k) map.q[qo + k] = (uint16_t)(fi + k);
+      for (int k = 0; k < 6; ++k) { map.qd[vo + k] = (uint16_t)(fi + 7 + k); map.qdd[vo + k] = (uint16_t)(fi + 13 + k); }
+    } else if (m.jtype[i] != BARD_JOINT_FIXED) {
+      map.q[qo] = (uint16_t)(reg + 6); map.qd[vo] = (uint16_t)reg; map.qdd[vo] = (uint16_t)(reg + 1);
+    }
+  }
   auto go = [&](auto kernel, auto id) {
     bard_status s = prep<decltype(id)::value>(kernel, "bard_rnea");
     if (s != BARD_OK) return s;
     kernel<<<cfg.grid, cfg.threads, cfg.smem, (cudaStream_t)stream>>>(m.d_blob, (uint32_t)m.common_bytes, m.team_warps,
                                                                       cfg.rcpL, cfg.team_rows, m.nq, m.nv, m.nb, m.nslots,
-                                                                      (uint32_t)B, q, qd, qdd, tau);
+                                                                      (uint32_t)B, q, qd, qdd, tau, map);
     return finish("bard_rnea");
   };
   return BARD_DISPATCH(rnea_kernel, 8, m.simple, cfg.pack, go);

@@ -330,6 +330,7 @@ bard_status build_model(const bard_model_desc* d, int device, Model& M) {
   }
   BodyConst* BC = reinterpret_cast<BodyConst*>(M.blob.data() + sizeof(BlobHeader));
   M.rodrigues.assign((size_t)nb * 36, 0.f);
+  M.free_index.assign(nb, -1);
   for (int i = 0; i < nb; ++i) {
     BodyConst& c = BC[i];
     const int t = M.jtype[i];
@@ -391,7 +392,7 @@ bard_status build_model(const bard_model_desc* d, int device, Model& M) {
     put(c.Io, Io, 6);
     c.type = t; c.parent = M.parent[i]; c.q_off = M.q_off[i]; c.v_off = M.v_off[i];
     c.src = src[i]; c.save = save[i]; c.flags = post_id ? 1 : 0; c.level = M.body_level[i];
-    if (t == BARD_JOINT_FREE) c.flags |= (M.nfree++) << 8;
+    if (t == BARD_JOINT_FREE) { M.free_index[i] = M.nfree; c.flags |= (M.nfree++) << 8; }
     c.anc_lo = (uint32_t)M.anc_mask[i]; c.anc_hi = (uint32_t)(M.anc_mask[i] >> 32);
     c.child_begin = child_begin[i]; c.child_count = (int32_t)children[i].size();
   }
