@@ -259,6 +259,9 @@ __device__ __forceinline__ Ctx setup(const void* gcommon, uint32_t cbytes, const
   c.common = 4;
   c.extra = 4 + (cbytes >> 2);
   c.st = c.extra + (xbytes >> 2) + team * team_rows * RW + c.lane * N;
+  // Programmatic dependent launch: let the next kernel in the stream start its own prologue while this grid
+  // drains; our constants are immutable, so only the batched inputs wait for the previous grid (below).
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   if (threadIdx.x == 0) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar_a));
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -266,6 +269,7 @@ __device__ __forceinline__ Ctx setup(const void* gcommon, uint32_t cbytes, const
     bulk_g2s(bar_a + 16, gcommon, cbytes, bar_a);
     if (xbytes) bulk_g2s(bar_a + 16 + cbytes, gextra, xbytes, bar_a);
   }
+  asm volatile("griddepcontrol.wait;" ::: "memory");           // previous grid complete, its writes visible
   // stage the team's input rows; warp w takes rows w, w + L, ...
   const uint32_t st_a = bar_a + 4u * c.st;
   if (map) {
@@ -927,6 +931,23 @@ bard_status refuse(const char* name, const std::string& why) {
 }
 template <int V> using IC = std::integral_constant<int, V>;
 
+// Launch with programmatic stream serialization (PDL): see setup().
+template <typename K, typename... Args>
+void launch(K kernel, const LaunchCfg& cfg, void* stream, Args... args) {
+  static const int pdl = env_int("BARD_PDL", 1);
+  cudaLaunchConfig_t lc = {};
+  lc.gridDim = dim3(cfg.grid);
+  lc.blockDim = dim3(cfg.threads);
+  lc.dynamicSmemBytes = cfg.smem;
+  lc.stream = (cudaStream_t)stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  lc.attrs = attr;
+  lc.numAttrs = pdl ? 1 : 0;
+  cudaLaunchKernelEx(&lc, kernel, args...);
+}
+
 // Calls go(kernel<SIMPLE, N>, id) for the run-time (simple, pack) pair.
 #define BARD_DISPATCH(KERNEL, BASE, simple, pack, go)                                           \
   ((simple) ? ((pack) == 2 ? go(KERNEL<true, 2>, IC<BASE + 0>()) : go(KERNEL<true, 1>, IC<BASE + 1>()))   \
@@ -942,8 +963,8 @@ bard_status launch_fk(const Model& m, int64_t B, const float* q, float* pose, vo
   auto go = [&](auto kernel, auto id) {
     bard_status s = prep<decltype(id)::value>(kernel, "bard_fk");
     if (s != BARD_OK) return s;
-    kernel<<<cfg.grid, cfg.threads, cfg.smem, (cudaStream_t)stream>>>(m.d_blob, (uint32_t)m.common_bytes, m.team_warps,
-                                                                      cfg.rcpL, cfg.team_rows, m.nq, (uint32_t)B, q, pose);
+    launch(kernel, cfg, stream, (const void*)m.d_blob, (uint32_t)m.common_bytes, (int)m.team_warps, cfg.rcpL, cfg.team_rows,
+           (int)m.nq, (uint32_t)B, q, pose);
     return finish("bard_fk");
   };
   return BARD_DISPATCH(fk_kernel, 0, m.simple, cfg.pack, go);
@@ -959,9 +980,8 @@ bard_status launch_jacobian(const Model& m, int64_t B, const float* q, float* J,
   auto go = [&](auto kernel, auto id) {
     bard_status s = prep<decltype(id)::value>(kernel, "bard_jacobian");
     if (s != BARD_OK) return s;
-    kernel<<<cfg.grid, cfg.threads, cfg.smem, (cudaStream_t)stream>>>(
-        m.d_blob, (uint32_t)m.common_bytes, m.d_jblob, (uint32_t)m.j_bytes, m.team_warps, cfg.rcpL, cfg.team_rows, m.nq,
-        m.nv, m.nslots, (uint32_t)B, q, J, vec_ok);
+    launch(kernel, cfg, stream, (const void*)m.d_blob, (uint32_t)m.common_bytes, (const void*)m.d_jblob, (uint32_t)m.j_bytes,
+           (int)m.team_warps, cfg.rcpL, cfg.team_rows, (int)m.nq, (int)m.nv, (int)m.nslots, (uint32_t)B, q, J, vec_ok);
     return finish("bard_jacobian");
   };
   return BARD_DISPATCH(jacobian_kernel, 4, m.simple, cfg.pack, go);
@@ -987,9 +1007,8 @@ bard_status launch_rnea(const Model& m, int64_t B, const float* q, const float* 
   auto go = [&](auto kernel, auto id) {
     bard_status s = prep<decltype(id)::value>(kernel, "bard_rnea");
     if (s != BARD_OK) return s;
-    kernel<<<cfg.grid, cfg.threads, cfg.smem, (cudaStream_t)stream>>>(m.d_blob, (uint32_t)m.common_bytes, m.team_warps,
-                                                                      cfg.rcpL, cfg.team_rows, m.nq, m.nv, m.nb, m.nslots,
-                                                                      (uint32_t)B, q, qd, qdd, tau, map);
+    launch(kernel, cfg, stream, (const void*)m.d_blob, (uint32_t)m.common_bytes, (int)m.team_warps, cfg.rcpL, cfg.team_rows,
+           (int)m.nq, (int)m.nv, (int)m.nb, (int)m.nslots, (uint32_t)B, q, qd, qdd, tau, map);
     return finish("bard_rnea");
   };
   return BARD_DISPATCH(rnea_kernel, 8, m.simple, cfg.pack, go);
@@ -1005,9 +1024,8 @@ bard_status launch_crba(const Model& m, int64_t B, const float* q, float* M, voi
   auto go = [&](auto kernel, auto id) {
     bard_status s = prep<decltype(id)::value>(kernel, "bard_crba");
     if (s != BARD_OK) return s;
-    kernel<<<cfg.grid, cfg.threads, cfg.smem, (cudaStream_t)stream>>>(
-        m.d_blob, (uint32_t)m.common_bytes, (uint32_t)m.m_bytes, m.crba_warps, cfg.rcpL, cfg.team_rows, m.nq, m.nv,
-        m.nslots, (uint32_t)B, q, M, vec_ok);
+    launch(kernel, cfg, stream, (const void*)m.d_blob, (uint32_t)m.common_bytes, (uint32_t)m.m_bytes, (int)m.crba_warps, cfg.rcpL,
+           cfg.team_rows, (int)m.nq, (int)m.nv, (int)m.nslots, (uint32_t)B, q, M, vec_ok);
     return finish("bard_crba");
   };
   return BARD_DISPATCH(crba_kernel, 12, m.simple, cfg.pack, go);
