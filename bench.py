@@ -219,6 +219,31 @@ def time_op_train(torch, m, op, sets, B, stream, launches, warm=5):
     return e0.elapsed_time(e1) * 1e-3 / launches
 
 
+def time_op_graph(torch, m, op, sets, B, launches=64, replays=10):
+    """Same train captured once into a CUDA graph and replayed: device-side time per launch without the host's
+    per-call cost (at B = 4096 a launch through ctypes costs more than the kernel)."""
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        for i in range(4):
+            op_call(m, op, sets[i % len(sets)], B, side.cuda_stream)
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=side):
+        for i in range(launches):
+            op_call(m, op, sets[i % len(sets)], B, side.cuda_stream)
+    g.replay()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(replays):
+        g.replay()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) * 1e-3 / (launches * replays)
+
+
 def op_report(desc, pk, op, sec, B):
     r = RL.roofline(desc, pk)[op]
     if r["bound"] == "hbm":
@@ -307,6 +332,12 @@ def run_ours(args):
             sec = time_op_train(torch, m, op, sets_s, 4096, stream, launches=200)
             r = op_report(desc, pk, op, sec, 4096)
             small[op] = {k: r[k] for k in ("us", "env_evals_per_s", "bound", "frac")}
+            try:
+                secg = time_op_graph(torch, m, op, sets_s, 4096)
+                rg = op_report(desc, pk, op, secg, 4096)
+                small[op]["cuda_graph"] = {k: rg[k] for k in ("us", "env_evals_per_s", "frac")}
+            except Exception as ex:                      # graph capture is a convenience of the bench, not of the path
+                small[op]["cuda_graph"] = {"error": str(ex)[:120]}
         del sets_s
     clocks.active.clear()
 
