@@ -728,66 +728,73 @@ __global__ void __launch_bounds__(256) crba_kernel(const void* __restrict__ gcom
   const int dof = slots + nslots * 12 * RW;                    // 6 rows per DOF
   const int ic = dof + nv * 6 * RW;                            // 10 rows per body: m h(3) I(6)
   const int fpose = ic + ldci(C.common + H_NB) * 10 * RW;      // 12 rows per free-joint body: R p
-  Pose<T> cur;
-  int ntask = 0;
-  for (int k = 0;; ++k) {
-    const uint32_t tk = ldc_u16(C.tasks_b + 2 * k);
-    if (tk == TASK_END) { ntask = k; break; }
-    if (!(tk & TASK_NOOP)) {
-      const int i = tk & TASK_BODY_MASK;
-      const int body = C.bodies + 64 * i;
-      const Meta m = load_meta(body);
-      T u, w;
-      fk_body<SIMPLE, T, RW>(body, m, qs, slots, cur, u, w);
-      store_screws<SIMPLE, T, RW>(body, m, cur, dof);
-      if (m.type == BARD_JOINT_FREE) {
-        const int fp = fpose + ((m.flags >> 8) & 0xff) * 12 * RW;
-#pragma unroll
-        for (int j = 0; j < 9; ++j) sts(fp + j * RW, cur.R.m[j]);
-        strow3<RW>(fp + 9 * RW, cur.p);
+  if (C.w >= ldci(C.common + 5)) {
+    // helper warp (w >= L): no body of its own in the level sweeps, only the team barriers -- nlevels in the
+    // outward sweep, nlevels - 1 in the inward one -- then its share of the fill
+    const int nl = ldci(C.common + 3);
+    for (int l = 0; l < 2 * nl - 1; ++l) team_sync(C);
+  } else {
+    Pose<T> cur;
+    int ntask = 0;
+    for (int k = 0;; ++k) {
+      const uint32_t tk = ldc_u16(C.tasks_b + 2 * k);
+      if (tk == TASK_END) { ntask = k; break; }
+      if (!(tk & TASK_NOOP)) {
+        const int i = tk & TASK_BODY_MASK;
+        const int body = C.bodies + 64 * i;
+        const Meta m = load_meta(body);
+        T u, w;
+        fk_body<SIMPLE, T, RW>(body, m, qs, slots, cur, u, w);
+        store_screws<SIMPLE, T, RW>(body, m, cur, dof);
+        if (m.type == BARD_JOINT_FREE) {
+          const int fp = fpose + ((m.flags >> 8) & 0xff) * 12 * RW;
+  #pragma unroll
+          for (int j = 0; j < 9; ++j) sts(fp + j * RW, cur.R.m[j]);
+          strow3<RW>(fp + 9 * RW, cur.p);
+        }
+        // body inertia about the world origin: h' = R h + m p ; with h'' = R h + m p / 2:
+        // I' = R Io R^T + 2 (p . h'') 1 - (h'' p^T + p h''^T)
+        const Inertia in = load_inertia(body);
+        const float ms = in.mass;
+        const V3<T> p = cur.p;
+        const V3<T> hr = mul(cur.R, in.h);
+        const V3<T> hh = axpy(0.5f * ms, p, hr);
+        const V3<T> r0 = {cur.R.m[0], cur.R.m[1], cur.R.m[2]}, r1 = {cur.R.m[3], cur.R.m[4], cur.R.m[5]},
+                    r2 = {cur.R.m[6], cur.R.m[7], cur.R.m[8]};
+        const V3<T> a0 = symmul(in.Io, r0), a1 = symmul(in.Io, r1), a2 = symmul(in.Io, r2);
+        const T d = T(2.f) * dot(p, hh);
+        const int o = ic + i * 10 * RW;
+        sts(o, T(ms));
+        strow3<RW>(o + RW, axpy(ms, p, hr));
+        sts(o + 4 * RW, fm(T(-2.f) * hh.x, p.x, dot_acc(r0, a0, d)));           // xx
+        sts(o + 5 * RW, fm(-hh.x, p.y, fm(-p.x, hh.y, dot(r0, a1))));           // xy
+        sts(o + 6 * RW, fm(-hh.x, p.z, fm(-p.x, hh.z, dot(r0, a2))));           // xz
+        sts(o + 7 * RW, fm(T(-2.f) * hh.y, p.y, dot_acc(r1, a1, d)));           // yy
+        sts(o + 8 * RW, fm(-hh.y, p.z, fm(-p.y, hh.z, dot(r1, a2))));           // yz
+        sts(o + 9 * RW, fm(T(-2.f) * hh.z, p.z, dot_acc(r2, a2, d)));           // zz
       }
-      // body inertia about the world origin: h' = R h + m p ; with h'' = R h + m p / 2:
-      // I' = R Io R^T + 2 (p . h'') 1 - (h'' p^T + p h''^T)
-      const Inertia in = load_inertia(body);
-      const float ms = in.mass;
-      const V3<T> p = cur.p;
-      const V3<T> hr = mul(cur.R, in.h);
-      const V3<T> hh = axpy(0.5f * ms, p, hr);
-      const V3<T> r0 = {cur.R.m[0], cur.R.m[1], cur.R.m[2]}, r1 = {cur.R.m[3], cur.R.m[4], cur.R.m[5]},
-                  r2 = {cur.R.m[6], cur.R.m[7], cur.R.m[8]};
-      const V3<T> a0 = symmul(in.Io, r0), a1 = symmul(in.Io, r1), a2 = symmul(in.Io, r2);
-      const T d = T(2.f) * dot(p, hh);
-      const int o = ic + i * 10 * RW;
-      sts(o, T(ms));
-      strow3<RW>(o + RW, axpy(ms, p, hr));
-      sts(o + 4 * RW, fm(T(-2.f) * hh.x, p.x, dot_acc(r0, a0, d)));           // xx
-      sts(o + 5 * RW, fm(-hh.x, p.y, fm(-p.x, hh.y, dot(r0, a1))));           // xy
-      sts(o + 6 * RW, fm(-hh.x, p.z, fm(-p.x, hh.z, dot(r0, a2))));           // xz
-      sts(o + 7 * RW, fm(T(-2.f) * hh.y, p.y, dot_acc(r1, a1, d)));           // yy
-      sts(o + 8 * RW, fm(-hh.y, p.z, fm(-p.y, hh.z, dot(r1, a2))));           // yz
-      sts(o + 9 * RW, fm(T(-2.f) * hh.z, p.z, dot_acc(r2, a2, d)));           // zz
+      if (tk & TASK_BAR) team_sync(C);
     }
-    if (tk & TASK_BAR) team_sync(C);
-  }
-  // composite sweep, deepest level first
-  for (int k = ntask - 1; k >= 0; --k) {
-    const uint32_t tk = ldc_u16(C.tasks_b + 2 * k);
-    if ((tk & TASK_BAR) && k != ntask - 1) team_sync(C);
-    if (tk & TASK_NOOP) continue;
-    const int i = tk & TASK_BODY_MASK;
-    const int cbeg = ldci(C.bodies + 64 * i + 62), ccnt = ldci(C.bodies + 64 * i + 63);
-    if (ccnt == 0) continue;
-    const int d = ic + i * 10 * RW;
-    T acc[10];
-#pragma unroll
-    for (int j = 0; j < 10; ++j) acc[j] = lds<T>(d + j * RW);
-    for (int cc = 0; cc < ccnt; ++cc) {
-      const int s = ic + (int)ldc_u8(children_b + cbeg + cc) * 10 * RW;
-#pragma unroll
-      for (int j = 0; j < 10; ++j) acc[j] = acc[j] + lds<T>(s + j * RW);
+    // composite sweep, deepest level first
+    for (int k = ntask - 1; k >= 0; --k) {
+      const uint32_t tk = ldc_u16(C.tasks_b + 2 * k);
+      if ((tk & TASK_BAR) && k != ntask - 1) team_sync(C);
+      if (tk & TASK_NOOP) continue;
+      const int i = tk & TASK_BODY_MASK;
+      const int cbeg = ldci(C.bodies + 64 * i + 62), ccnt = ldci(C.bodies + 64 * i + 63);
+      if (ccnt == 0) continue;
+      const int d = ic + i * 10 * RW;
+      T acc[10];
+  #pragma unroll
+      for (int j = 0; j < 10; ++j) acc[j] = lds<T>(d + j * RW);
+      for (int cc = 0; cc < ccnt; ++cc) {
+        const int s = ic + (int)ldc_u8(children_b + cbeg + cc) * 10 * RW;
+  #pragma unroll
+        for (int j = 0; j < 10; ++j) acc[j] = acc[j] + lds<T>(s + j * RW);
+      }
+  #pragma unroll
+      for (int j = 0; j < 10; ++j) sts(d + j * RW, acc[j]);
     }
-#pragma unroll
-    for (int j = 0; j < 10; ++j) sts(d + j * RW, acc[j]);
   }
   team_sync(C);
   // fill

@@ -202,3 +202,17 @@ def test_too_many_elements_is_refused_not_wrapped():
     with pytest.raises(binding.BardError) as e:
         m.crba(1 << 23, t, t)                      # 841 * 2^23 > 2^32: refused before any launch
     assert e.value.code == 3
+
+
+@pytest.mark.parametrize("cfg", [1, 3])
+def test_repeated_launches_are_bit_identical(cfg):
+    """No atomics, fixed child order (DESIGN reading 7): every launch must reproduce the same bits.  A race
+    between a team's warps (barriers, shared-memory rows that are reused) would show up here as noise."""
+    desc = W.config_robot(cfg)
+    g = Gpu(desc)
+    q, qd, qdd = W.config_states(cfg, 4096 + 32)
+    ref = g.run(q, qd, qdd)
+    for _ in range(5):
+        out = g.run(q, qd, qdd)
+        for a, b in zip(ref, out):
+            assert np.array_equal(a, b)
