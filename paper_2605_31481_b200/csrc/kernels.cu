@@ -40,22 +40,27 @@ extern std::atomic<int64_t> g_launches;
 namespace {
 
 // ----------------------------------------------------------------------------- scalar packs
-// f2: the same quantity for the lane's two environments.  A plain float converts to an f2 with both halves
-// equal (a model constant), so mixed expressions need no extra overloads.
+// f2: the same quantity for the lane's two environments, kept in one aligned 64-bit register pair so that the
+// arithmetic maps onto Blackwell's packed FP32 instructions (PTX add / mul / fma .f32x2 -> SASS FADD2 / FMUL2 /
+// FFMA2): one issue slot does the work of two, and the kernels are bound by instruction issue.  A plain float
+// converts to an f2 with both halves equal (a model constant: FFMA2 reads it as a broadcast `.F32` operand, no
+// extra instruction), so mixed expressions need no extra overloads.
 struct f2 {
-  float a, b;
+  unsigned long long v;
   __device__ __forceinline__ f2() {}
-  __device__ __forceinline__ f2(float s) : a(s), b(s) {}
-  __device__ __forceinline__ f2(float x, float y) : a(x), b(y) {}
+  __device__ __forceinline__ f2(float x, float y) { asm("mov.b64 %0, {%1, %2};" : "=l"(v) : "f"(x), "f"(y)); }
+  __device__ __forceinline__ f2(float s) : f2(s, s) {}
+  __device__ __forceinline__ float lo() const { float x, y; asm("mov.b64 {%0, %1}, %2;" : "=f"(x), "=f"(y) : "l"(v)); return x; }
+  __device__ __forceinline__ float hi() const { float x, y; asm("mov.b64 {%0, %1}, %2;" : "=f"(x), "=f"(y) : "l"(v)); return y; }
 };
-__device__ __forceinline__ f2 operator+(f2 x, f2 y) { return {x.a + y.a, x.b + y.b}; }
-__device__ __forceinline__ f2 operator-(f2 x, f2 y) { return {x.a - y.a, x.b - y.b}; }
-__device__ __forceinline__ f2 operator*(f2 x, f2 y) { return {x.a * y.a, x.b * y.b}; }
-__device__ __forceinline__ f2 operator-(f2 x) { return {-x.a, -x.b}; }
+__device__ __forceinline__ f2 operator-(f2 x) { return {-x.lo(), -x.hi()}; }     // folds into an operand modifier
+__device__ __forceinline__ f2 operator+(f2 x, f2 y) { f2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(x.v), "l"(y.v)); return r; }
+__device__ __forceinline__ f2 operator-(f2 x, f2 y) { return x + (-y); }
+__device__ __forceinline__ f2 operator*(f2 x, f2 y) { f2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(x.v), "l"(y.v)); return r; }
 __device__ __forceinline__ float fm(float x, float y, float z) { return fmaf(x, y, z); }
-__device__ __forceinline__ f2 fm(f2 x, f2 y, f2 z) { return {fmaf(x.a, y.a, z.a), fmaf(x.b, y.b, z.b)}; }
+__device__ __forceinline__ f2 fm(f2 x, f2 y, f2 z) { f2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r.v) : "l"(x.v), "l"(y.v), "l"(z.v)); return r; }
 __device__ __forceinline__ float rsq(float x) { return rsqrtf(x); }
-__device__ __forceinline__ f2 rsq(f2 x) { return {rsqrtf(x.a), rsqrtf(x.b)}; }
+__device__ __forceinline__ f2 rsq(f2 x) { return {rsqrtf(x.lo()), rsqrtf(x.hi())}; }
 
 template <int N> struct Pack { using T = float; };
 template <> struct Pack<2> { using T = f2; };
@@ -149,8 +154,24 @@ __device__ __forceinline__ void sincos_fast(float x, float& s, float& c) {
   c = __int_as_float(__float_as_int(cc) ^ (((qd + 1) & 2) << 30));
 }
 __device__ __forceinline__ void sincos_fast(f2 x, f2& s, f2& c) {
-  sincos_fast(x.a, s.a, c.a);
-  sincos_fast(x.b, s.b, c.b);
+  // same arithmetic as the scalar version, the FP part in packed form; the quadrant logic stays per half
+  const f2 kb = fm(x, f2(0.636619772367581343f), f2(12582912.0f));
+  const f2 k = kb + f2(-12582912.0f);
+  const int q0 = __float_as_int(kb.lo()), q1 = __float_as_int(kb.hi());
+  f2 r = fm(k, f2(-1.57079637050628662109375f), x);
+  r = fm(k, f2(4.371138828673793e-8f), r);
+  r = fm(k, f2(1.7151245100058819e-15f), r);
+  const f2 r2 = r * r;
+  f2 ps = fm(r2, f2(-1.9515295891e-4f), f2(8.3321608736e-3f));
+  ps = fm(ps, r2, f2(-1.6666654611e-1f));
+  ps = fm(ps * r2, r, r);
+  f2 pc = fm(r2, f2(2.443315711809948e-5f), f2(-1.388731625493765e-3f));
+  pc = fm(pc, r2, f2(4.166664568298827e-2f));
+  pc = fm(pc * r2, r2, fm(r2, f2(-0.5f), f2(1.0f)));
+  const float ss0 = (q0 & 1) ? pc.lo() : ps.lo(), cc0 = (q0 & 1) ? ps.lo() : pc.lo();
+  const float ss1 = (q1 & 1) ? pc.hi() : ps.hi(), cc1 = (q1 & 1) ? ps.hi() : pc.hi();
+  s = {__int_as_float(__float_as_int(ss0) ^ ((q0 & 2) << 30)), __int_as_float(__float_as_int(ss1) ^ ((q1 & 2) << 30))};
+  c = {__int_as_float(__float_as_int(cc0) ^ (((q0 + 1) & 2) << 30)), __int_as_float(__float_as_int(cc1) ^ (((q1 + 1) & 2) << 30))};
 }
 
 // ----------------------------------------------------------------------------- shared memory, staging, addressing
@@ -162,11 +183,12 @@ extern __shared__ __align__(16) float smf[];
 template <class T> __device__ __forceinline__ T lds(int idx);
 template <> __device__ __forceinline__ float lds<float>(int idx) { return smf[idx]; }
 template <> __device__ __forceinline__ f2 lds<f2>(int idx) {
-  const float2 v = *reinterpret_cast<const float2*>(smf + idx);
-  return {v.x, v.y};
+  f2 r;
+  r.v = *reinterpret_cast<const unsigned long long*>(smf + idx);
+  return r;
 }
 __device__ __forceinline__ void sts(int idx, float v) { smf[idx] = v; }
-__device__ __forceinline__ void sts(int idx, f2 v) { *reinterpret_cast<float2*>(smf + idx) = make_float2(v.a, v.b); }
+__device__ __forceinline__ void sts(int idx, f2 v) { *reinterpret_cast<unsigned long long*>(smf + idx) = v.v; }
 // three consecutive state rows (RW floats apart) starting at idx
 template <class T, int RW> __device__ __forceinline__ V3<T> ldrow3(int idx) {
   return {lds<T>(idx), lds<T>(idx + RW), lds<T>(idx + 2 * RW)};
@@ -185,7 +207,7 @@ __device__ __forceinline__ uint32_t ldc_u8(int byte_off) { return reinterpret_ca
 // global stores of a pack at a 32-bit element index (streaming: outputs are never re-read by the kernels)
 __device__ __forceinline__ void stg(float* out, uint32_t idx, float v) { __stcs(out + idx, v); }
 __device__ __forceinline__ void stg(float* out, uint32_t idx, f2 v) {
-  __stcs(reinterpret_cast<float2*>(out + idx), make_float2(v.a, v.b));
+  __stcs(reinterpret_cast<unsigned long long*>(out + idx), v.v);
 }
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
