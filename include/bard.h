@@ -104,6 +104,23 @@ bard_status bard_model_get_table(const bard_model* m, int table_id, void* host_d
  * [nframes*3], NULL = zeros).  Not thread-safe against concurrent bard_jacobian calls. */
 bard_status bard_model_set_frames(bard_model* m, int32_t nframes, const int32_t* body, const double* offset);
 
+/* Operators, as bits of the `ops` mask of bard_model_specialize. */
+enum { BARD_OP_FK = 1, BARD_OP_JACOBIAN = 2, BARD_OP_RNEA = 4, BARD_OP_CRBA = 8 };
+
+/* Model-specialised kernels (optional, once per model, takes seconds): writes straight-line CUDA source of
+ * the operators in `ops` for THIS model -- constants as literals, the tree walked depth first so that the
+ * inward pass of a subtree follows its outward pass (eq. (6)) and only the bodies on
+ * the current root-to-leaf path hold parked state -- compiles it for sm_100a with NVRTC (libnvrtc.so.12 of the
+ * CUDA toolkit, loaded with dlopen) and loads the cubin.  Afterwards bard_<op> calls with a large batch
+ * (B >= 16384) launch the specialised kernel, smaller ones the level-parallel team kernel; results agree to
+ * rounding.  Only BARD_OP_RNEA has a generator so far: any other bit returns BARD_ERR_UNSUPPORTED.  On a
+ * host-only model the source is generated and compiled but not loaded.  NVRTC missing or a compile error:
+ * BARD_ERR_CUDA with the log in bard_last_error; the model stays usable.  Not thread-safe against concurrent
+ * operator calls on the same model. */
+bard_status bard_model_specialize(bard_model* m, uint32_t ops);
+/* The generated source of one specialised operator (NUL-terminated) into host_dst; query with cap 0. */
+bard_status bard_model_specialized_source(const bard_model* m, uint32_t op, char* host_dst, size_t cap, size_t* need);
+
 /* FK (eq. (1)-(5), level-ordered outward propagation). */
 bard_status bard_fk(const bard_model* m, int64_t B, const float* q, float* pose, bard_stream stream);
 /* Geometric Jacobian of the frames chosen by bard_model_set_frames (eq. (7)). */

@@ -20,11 +20,12 @@ from . import build as _build
 BARD_OK = 0
 STATUS = {0: "BARD_OK", 1: "BARD_ERR_INVALID_ARG", 2: "BARD_ERR_TOPOLOGY", 3: "BARD_ERR_UNSUPPORTED",
           4: "BARD_ERR_ALLOC", 5: "BARD_ERR_CUDA"}
+OPS = {"fk": 1, "jacobian": 2, "rnea": 4, "crba": 8}
 TABLES = {"LEVEL_PTR": (0, np.int32), "LEVEL_BODY": (1, np.int32), "BODY_LEVEL": (2, np.int32),
           "PARENT_SLOT": (3, np.int32), "Q_OFF": (4, np.int32), "V_OFF": (5, np.int32), "DOF_BODY": (6, np.int32),
           "ANC_MASK": (7, np.uint64), "RODRIGUES": (8, np.float32)}
 EXPORTS = ["bard_model_create", "bard_model_destroy", "bard_model_dims", "bard_model_get_table",
-           "bard_model_set_frames", "bard_fk", "bard_jacobian", "bard_rnea", "bard_crba",
+           "bard_model_set_frames", "bard_model_specialize", "bard_model_specialized_source", "bard_fk", "bard_jacobian", "bard_rnea", "bard_crba",
            "bard_status_string", "bard_last_error", "bard_launch_count"]
 
 
@@ -59,6 +60,8 @@ def lib():
         L.bard_model_dims.argtypes = [vp] + [C.POINTER(C.c_int32)] * 4
         L.bard_model_get_table.argtypes = [vp, C.c_int, vp, C.c_size_t, C.POINTER(C.c_size_t)]
         L.bard_model_set_frames.argtypes = [vp, C.c_int32, C.POINTER(C.c_int32), C.POINTER(C.c_double)]
+        L.bard_model_specialize.argtypes = [vp, C.c_uint32]
+        L.bard_model_specialized_source.argtypes = [vp, C.c_uint32, C.c_char_p, C.c_size_t, C.POINTER(C.c_size_t)]
         L.bard_fk.argtypes = [vp, i64, fp, fp, vp]
         L.bard_jacobian.argtypes = [vp, i64, fp, fp, vp]
         L.bard_rnea.argtypes = [vp, i64, fp, fp, fp, fp, vp]
@@ -150,6 +153,20 @@ class Model:
         _check(lib().bard_model_set_frames(self._h, len(body), body.ctypes.data_as(C.POINTER(C.c_int32)),
                                            _dp(off) if off is not None else None))
         self.nframes = len(body)
+
+    def specialize(self, ops=("rnea",)):
+        """JIT-compile model-specialised kernels for the named operators (``bard_model_specialize``)."""
+        mask = 0
+        for o in ops:
+            mask |= OPS[o]
+        _check(lib().bard_model_specialize(self._h, mask))
+
+    def specialized_source(self, op: str) -> str:
+        need = C.c_size_t()
+        lib().bard_model_specialized_source(self._h, OPS[op], None, 0, C.byref(need))
+        buf = C.create_string_buffer(max(need.value, 1))
+        _check(lib().bard_model_specialized_source(self._h, OPS[op], buf, need.value, C.byref(need)))
+        return buf.value.decode()
 
     def table(self, name: str) -> np.ndarray:
         tid, dt = TABLES[name]

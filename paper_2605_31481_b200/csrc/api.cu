@@ -43,6 +43,7 @@ void bard_model_destroy(bard_model* bm) {
     if (bm->m.d_jblob) cudaFree(bm->m.d_jblob);
     cudaSetDevice(prev);
   }
+  bard::free_specialized(bm->m.spec);
   delete bm;
 }
 
@@ -87,6 +88,21 @@ bard_status bard_model_set_frames(bard_model* bm, int32_t nframes, const int32_t
   return bard::set_frames(bm->m, nframes, body, offset);
 }
 
+bard_status bard_model_specialize(bard_model* bm, uint32_t ops) {
+  if (!bm) { set_error("bard_model_specialize: model is NULL"); return BARD_ERR_INVALID_ARG; }
+  return bard::specialize(bm->m, ops);
+}
+
+bard_status bard_model_specialized_source(const bard_model* bm, uint32_t op, char* host_dst, size_t cap, size_t* need) {
+  if (!bm) { set_error("bard_model_specialized_source: model is NULL"); return BARD_ERR_INVALID_ARG; }
+  const std::string* src = bard::specialized_source(bm->m, op);
+  if (!src) { set_error("bard_model_specialized_source: operator not specialised"); return BARD_ERR_INVALID_ARG; }
+  if (need) *need = src->size() + 1;
+  if (cap < src->size() + 1 || !host_dst) { set_error("bard_model_specialized_source: destination too small"); return BARD_ERR_INVALID_ARG; }
+  std::memcpy(host_dst, src->c_str(), src->size() + 1);
+  return BARD_OK;
+}
+
 static bard_status check_call(const char* fn, const bard_model* bm, int64_t B, const void* a, const void* b,
                               const void* c, const void* d) {
   if (!bm) { set_error(std::string(fn) + ": model is NULL"); return BARD_ERR_INVALID_ARG; }
@@ -116,6 +132,7 @@ bard_status bard_rnea(const bard_model* bm, int64_t B, const float* q, const flo
   if (bm && bm->m.nv == 0) return check_call("bard_rnea", bm, B, bm, bm, bm, bm);  // nothing to write
   bard_status s = check_call("bard_rnea", bm, B, q, qd, qdd, tau);
   if (s != BARD_OK || B == 0) return s;
+  if (bard::launch_rnea_specialized(bm->m, B, q, qd, qdd, tau, stream, s)) return s;
   return bard::launch_rnea(bm->m, B, q, qd, qdd, tau, stream);
 }
 

@@ -96,8 +96,11 @@ struct JHeader {              // 8 words; byte offsets from the start of the J s
   int32_t off_bframes;        // uint16 [nb]: bit f set <=> frame f is attached to this body
 };
 
+struct Specialized;           // specialize.cu: model-specialised (NVRTC) kernels
+
 struct Model {
   int device = 0;
+  Specialized* spec = nullptr;
   int32_t nb = 0, nq = 0, nv = 0, nlevels = 0, nslots = 0, nframes = 0, nfree = 0;
   int32_t team_warps = 1;             // L: warps that share one 32-environment tile (level-parallel schedule)
   int32_t crba_warps = 1;             // Lc >= L: CRBA adds warps that only join the fill of M
@@ -127,5 +130,13 @@ bard_status launch_jacobian(const Model& m, int64_t B, const float* q, float* J,
 bard_status launch_rnea(const Model& m, int64_t B, const float* q, const float* qd, const float* qdd, float* tau,
                         void* stream);
 bard_status launch_crba(const Model& m, int64_t B, const float* q, float* M, void* stream);
+
+
+// specialize.cu
+bard_status specialize(Model& M, uint32_t ops);
+void free_specialized(Specialized* s);
+const std::string* specialized_source(const Model& M, uint32_t op);
+bool launch_rnea_specialized(const Model& M, int64_t B, const float* q, const float* qd, const float* qdd, float* tau,
+                             void* stream, bard_status& st);
 
 }  // namespace bard
