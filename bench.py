@@ -33,6 +33,7 @@ from paper_2605_31481_b200 import roofline as RL            # noqa: E402
 from paper_2605_31481_b200 import workloads as W            # noqa: E402
 
 OPS = ("fk", "jacobian", "rnea", "crba")
+SPEC_OPS = ("rnea",)
 METRIC = "env_evals_per_s (FK + Jacobian + RNEA + CRBA per environment)"
 UNIT = "env-evals/s"
 L2_BYTES = 126 * 1024 * 1024
@@ -48,6 +49,8 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--sweep", action="store_true", help="also time every operator over config 4's batch sweep")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-specialize", action="store_true",
+                    help="skip bard_model_specialize: every operator runs its table-driven team kernel")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU work for the oracle baseline")
     return ap.parse_args()
 
@@ -278,6 +281,8 @@ def run_ours(args):
     cfg, B, K, Wm = args.config, args.B, args.steps, max(args.warmup, 3)
     desc = W.config_robot(cfg)
     m = binding.Model(desc, device=local)
+    if not args.no_specialize:
+        m.specialize(SPEC_OPS)          # model-specialised (NVRTC) kernels for the operators that have a generator
     pk = RL.measured_peaks(ROOT)
     sets, per_set = make_sets(torch, m, desc, cfg, B, dev)
     R = len(sets)
@@ -396,11 +401,12 @@ def run_ours(args):
         "config": {"workload": workload_name(cfg, B), "envs_per_gpu": B, "global_envs": world * B,
                    "parallelism": f"batch-sharded x{world}, no collective",
                    "l2": f"{R} rotating buffer sets of {per_set / 1e6:.1f} MB (total {R * per_set / 1e6:.0f} MB > L2 126 MB)",
-                   "layout": "SoA batch-fastest"},
+                   "layout": "SoA batch-fastest",
+                   "specialized_ops": [] if args.no_specialize else list(SPEC_OPS)},
         "roofline": roof, "ops": ops, "ops_at_B4096": small, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks.summary(),
     }
     if args.sweep and rank == 0:
-        line["sweep"] = sweep(torch, binding, pk, dev, stream)
+        line["sweep"] = sweep(torch, binding, pk, dev, stream, specialize=not args.no_specialize)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cb, _, _ = time_oracle(desc, cfg, args.cpu_seconds)
         line["cpu_baseline"] = cb
@@ -410,12 +416,14 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
-def sweep(torch, binding, pk, dev, stream):
+def sweep(torch, binding, pk, dev, stream, specialize=True):
     """config 4: every operator on the humanoid and the chain at B = 1024 ... 1 048 576 (train timing)."""
     out = {}
     for cfg in (3, 0):
         desc = W.config_robot(cfg)
         m = binding.Model(desc, device=dev.index or 0)
+        if specialize:
+            m.specialize(SPEC_OPS)
         for B in (1024, 4096, 16384, 65536, 262144, 1048576):
             sets, _ = make_sets(torch, m, desc, cfg, B, dev, cap_bytes=40 << 30)
             row = {}

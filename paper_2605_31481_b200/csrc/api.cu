@@ -140,6 +140,7 @@ bard_status bard_crba(const bard_model* bm, int64_t B, const float* q, float* M,
   if (bm && bm->m.nv == 0) return check_call("bard_crba", bm, B, bm, bm, bm, bm);
   bard_status s = check_call("bard_crba", bm, B, q, M, M, M);
   if (s != BARD_OK || B == 0) return s;
+  if (bard::launch_crba_specialized(bm->m, B, q, M, stream, s)) return s;
   return bard::launch_crba(bm->m, B, q, M, stream);
 }
 

@@ -138,5 +138,6 @@ void free_specialized(Specialized* s);
 const std::string* specialized_source(const Model& M, uint32_t op);
 bool launch_rnea_specialized(const Model& M, int64_t B, const float* q, const float* qd, const float* qdd, float* tau,
                              void* stream, bard_status& st);
+bool launch_crba_specialized(const Model& M, int64_t B, const float* q, float* Mo, void* stream, bard_status& st);
 
 }  // namespace bard

@@ -60,7 +60,7 @@ def test_parked_rows_follow_the_path_not_the_body_count():
 def test_unsupported_operator_bits_are_refused():
     m = binding.Model(W.config_robot(0), device=-1)
     with pytest.raises(binding.BardError) as e:
-        m.specialize(("crba",))
+        m.specialize(("fk",))
     assert e.value.code == 3
     with pytest.raises(binding.BardError):
         m.specialized_source("rnea")                              # not specialised yet
