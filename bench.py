@@ -33,7 +33,7 @@ from paper_2605_31481_b200 import roofline as RL            # noqa: E402
 from paper_2605_31481_b200 import workloads as W            # noqa: E402
 
 OPS = ("fk", "jacobian", "rnea", "crba")
-SPEC_OPS = ("rnea",)
+SPEC_OPS = ("fk", "jacobian", "rnea", "crba")
 METRIC = "env_evals_per_s (FK + Jacobian + RNEA + CRBA per environment)"
 UNIT = "env-evals/s"
 L2_BYTES = 126 * 1024 * 1024

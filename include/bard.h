@@ -112,9 +112,10 @@ enum { BARD_OP_FK = 1, BARD_OP_JACOBIAN = 2, BARD_OP_RNEA = 4, BARD_OP_CRBA = 8 
  * inward pass of a subtree follows its outward pass (eq. (6)) and only the bodies on
  * the current root-to-leaf path hold parked state -- compiles it for sm_100a with NVRTC (libnvrtc.so.12 of the
  * CUDA toolkit, loaded with dlopen) and loads the cubin.  Afterwards bard_<op> calls with a large batch
- * (B >= 16384) launch the specialised kernel, smaller ones the level-parallel team kernel; results agree to
- * rounding.  Only BARD_OP_RNEA has a generator so far: any other bit returns BARD_ERR_UNSUPPORTED.  On a
- * host-only model the source is generated and compiled but not loaded.  NVRTC missing or a compile error:
+ * launch the specialised kernel (chains: any B; teams of <= 4 warps: B >= 4096; wider: B >= 32768), smaller ones
+ * the level-parallel team kernel; results agree to rounding.  The Jacobian is generated for the frames the
+ * model has at the time of the call: bard_model_set_frames drops it (specialise again afterwards).  Unknown
+ * bits: BARD_ERR_INVALID_ARG.  On a host-only model the source is generated and compiled but not loaded.  NVRTC missing or a compile error:
  * BARD_ERR_CUDA with the log in bard_last_error; the model stays usable.  Not thread-safe against concurrent
  * operator calls on the same model. */
 bard_status bard_model_specialize(bard_model* m, uint32_t ops);

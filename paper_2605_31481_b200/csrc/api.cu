@@ -85,6 +85,7 @@ bard_status bard_model_get_table(const bard_model* bm, int table_id, void* host_
 
 bard_status bard_model_set_frames(bard_model* bm, int32_t nframes, const int32_t* body, const double* offset) {
   if (!bm) { set_error("bard_model_set_frames: model is NULL"); return BARD_ERR_INVALID_ARG; }
+  bard::drop_specialized_jacobian(bm->m);
   return bard::set_frames(bm->m, nframes, body, offset);
 }
 
@@ -117,6 +118,7 @@ static bard_status check_call(const char* fn, const bard_model* bm, int64_t B, c
 bard_status bard_fk(const bard_model* bm, int64_t B, const float* q, float* pose, bard_stream stream) {
   bard_status s = check_call("bard_fk", bm, B, bm && bm->m.nq == 0 ? (const void*)pose : q, pose, pose, pose);
   if (s != BARD_OK || B == 0) return s;
+  if (bard::launch_fk_specialized(bm->m, B, q, pose, stream, s)) return s;
   return bard::launch_fk(bm->m, B, q, pose, stream);
 }
 
@@ -124,6 +126,7 @@ bard_status bard_jacobian(const bard_model* bm, int64_t B, const float* q, float
   if (bm && (bm->m.nframes == 0 || bm->m.nv == 0)) return check_call("bard_jacobian", bm, B, bm, bm, bm, bm);  // empty output
   bard_status s = check_call("bard_jacobian", bm, B, bm->m.nq == 0 ? (const void*)J : q, J, J, J);
   if (s != BARD_OK || B == 0) return s;
+  if (bard::launch_jacobian_specialized(bm->m, B, q, J, stream, s)) return s;
   return bard::launch_jacobian(bm->m, B, q, J, stream);
 }
 

@@ -1,5 +1,6 @@
 """Model-specialised kernels (bard_model_specialize): host-side generation + NVRTC compilation on CPU, and GPU
-parity of the generated RNEA against the fp64 oracle and against the level-parallel team kernel."""
+parity of the generated FK / Jacobian / RNEA / CRBA against the fp64 oracle and against the level-parallel
+team kernels."""
 import re
 
 import numpy as np
@@ -8,7 +9,8 @@ import pytest
 import oracle
 from paper_2605_31481_b200 import binding, workloads as W
 
-TOL_DYN = 1e-3
+TOL_KIN, TOL_DYN = 1e-4, 1e-3
+ALL = ("fk", "jacobian", "rnea", "crba")
 
 
 def nerr(x, ref):
@@ -19,7 +21,7 @@ def _robots():
     out = [W.config_robot(c) for c in range(4)]
     for seed in range(6):
         shape = ["random", "chain", "star", "unbalanced"][seed % 4]
-        out.append(W.random_tree(500 + seed, nb=2 + 4 * seed, shape=shape, free_root=(seed % 2 == 0)))
+        out.append(W.random_tree(500 + seed, nb=2 + 4 * seed, shape=shape, free_root=(seed % 2 == 0), nframes=3))
     return out
 
 
@@ -29,9 +31,14 @@ def test_generated_source_compiles_on_host(idx):
     """A host-only model: the source is generated and NVRTC-compiled for sm_100a, nothing is loaded."""
     desc = _robots()[idx]
     m = binding.Model(desc, device=-1)
-    m.specialize(("rnea",))
+    m.specialize(ALL)
+    for op in ALL:
+        assert 'extern "C" __global__' in m.specialized_source(op) and f"bard_{op}_n1" in m.specialized_source(op)
+    # FK: 12 rows per body; CRBA / Jacobian: every output row stored exactly once (fill + structural zeros)
+    for op, arr, n in (("fk", "pose", 12 * m.nb), ("crba", "Mo", m.nv * m.nv), ("jacobian", "J", 6 * m.nframes * m.nv)):
+        rows = sorted(int(r) for r in re.findall(r"strow\(%s, (\d+)u \* B \+ e" % arr, m.specialized_source(op)))
+        assert rows == list(range(n)), op
     src = m.specialized_source("rnea")
-    assert 'extern "C" __global__' in src and "bard_rnea_n1" in src
     # one outward and one inward section per body, every tau row stored exactly once
     assert len(re.findall(r"// ---- body \d+ \(outward\)", src)) == m.nb
     assert len(re.findall(r"// ---- body \d+ \(inward\)", src)) == m.nb
@@ -57,13 +64,18 @@ def test_parked_rows_follow_the_path_not_the_body_count():
     assert rows(W.config_robot(3)) <= 8 * 7 + 12 * 2 + 1          # humanoid: depth 7, two branch points on a path
 
 
-def test_unsupported_operator_bits_are_refused():
+def test_unknown_operator_bits_are_refused_and_set_frames_drops_the_jacobian():
     m = binding.Model(W.config_robot(0), device=-1)
-    with pytest.raises(binding.BardError) as e:
-        m.specialize(("fk",))
-    assert e.value.code == 3
+    assert binding.lib().bard_model_specialize(m._h, 1 << 7) == 1  # BARD_ERR_INVALID_ARG
     with pytest.raises(binding.BardError):
         m.specialized_source("rnea")                              # not specialised yet
+    m.specialize(("jacobian",))
+    assert "frame 0 on body 6" in m.specialized_source("jacobian")
+    m.set_frames([2])                                             # the generated code was for the old frame
+    with pytest.raises(binding.BardError):
+        m.specialized_source("jacobian")
+    m.specialize(("jacobian",))
+    assert "frame 0 on body 2" in m.specialized_source("jacobian")
 
 
 # ------------------------------------------------------------------------------------------- GPU
@@ -74,42 +86,61 @@ class Spec:
     def __init__(self, desc):
         assert torch.cuda.is_available(), "GPU tests need CUDA; there is no CPU fallback"
         self.m = binding.Model(desc, device=0)
-        self.m.specialize(("rnea",))
+        self.m.specialize(ALL)
         self.o = oracle.Oracle(desc)
         self.dev = torch.device("cuda:0")
 
-    def rnea(self, q, qd, qdd):
-        m, B = self.m, q.shape[1]
-        t = [torch.from_numpy(np.ascontiguousarray(a)).to(self.dev) for a in (q, qd, qdd)]
-        tau = torch.full((m.nv, B), float("nan"), device=self.dev)
+    def run(self, q, qd, qdd):
+        """All four operators, NaN-filled outputs (every element must be overwritten), one launch each."""
+        m, B, dev = self.m, q.shape[1], self.dev
+        tq, tqd, tqdd = (torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in (q, qd, qdd))
+        pose = torch.full((m.nb, 12, B), float("nan"), device=dev)
+        J = torch.full((m.nframes, 6, m.nv, B), float("nan"), device=dev)
+        tau = torch.full((m.nv, B), float("nan"), device=dev)
+        M = torch.full((m.nv, m.nv, B), float("nan"), device=dev)
+        s = torch.cuda.current_stream().cuda_stream
         n0 = binding.launch_count()
-        m.rnea(B, *t, tau, torch.cuda.current_stream().cuda_stream)
+        m.fk(B, tq, pose, s)
+        m.jacobian(B, tq, J, s)
+        m.rnea(B, tq, tqd, tqdd, tau, s)
+        m.crba(B, tq, M, s)
         torch.cuda.synchronize()
-        assert binding.launch_count() - n0 == 1
-        return tau.cpu().numpy()
+        assert binding.launch_count() - n0 == 4 or m.nv == 0 or m.nframes == 0   # one launch per operator
+        return pose.cpu().numpy(), J.cpu().numpy(), tau.cpu().numpy(), M.cpu().numpy()
+
+    def refs(self, q, qd, qdd):
+        q64, qd64, qdd64 = (np.ascontiguousarray(a.astype(np.float64)) for a in (q, qd, qdd))
+        J = self.o.jacobian(q64) if self.m.nframes else np.zeros((0, 6, self.m.nv, q.shape[1]))
+        return self.o.fk(q64), J, self.o.rnea(q64, qd64, qdd64), self.o.crba(q64)
+
+    def check(self, out, ref):
+        for a in out:
+            assert np.isfinite(a).all()
+        for a, r, tol in zip(out, ref, (TOL_KIN, TOL_KIN, TOL_DYN, TOL_DYN)):
+            assert nerr(a, r) <= tol
+        assert np.array_equal(out[3], np.swapaxes(out[3], 0, 1))   # M written symmetric, bit for bit
 
 
 @pytest.mark.gpu
 @pytest.mark.parametrize("idx", range(10))
 @pytest.mark.parametrize("B", [1, 37, 1000])
-def test_specialized_rnea_matches_oracle(idx, B, monkeypatch):
-    monkeypatch.setenv("BARD_SPEC_MIN_B", "0")                    # the specialised kernel at every batch size
+def test_specialized_operators_match_oracle(idx, B, monkeypatch):
+    monkeypatch.setenv("BARD_SPEC_MIN_B", "0")                    # the specialised kernels at every batch size
     desc = _robots()[idx]
     s = Spec(desc)
     q, qd, qdd = W.sample_states(desc, B, seed=900 + idx)
-    tau = s.rnea(q, qd, qdd)
-    assert np.isfinite(tau).all()
-    ref = s.o.rnea(*(a.astype(np.float64) for a in (q, qd, qdd)))
-    assert nerr(tau, ref) <= TOL_DYN
-    # and the team kernel on the same inputs: same arithmetic up to the folded zeros
+    out = s.run(q, qd, qdd)
+    s.check(out, s.refs(q, qd, qdd))
+    # and the team kernels on the same inputs: same arithmetic up to the folded zeros
     monkeypatch.setenv("BARD_SPEC_MIN_B", str(1 << 30))
-    team = s.rnea(q, qd, qdd)
-    assert nerr(tau, team.astype(np.float64)) <= 1e-4
+    team = s.run(q, qd, qdd)
+    for a, b in zip(out, team):
+        assert nerr(a, b.astype(np.float64)) <= 1e-4
 
 
 @pytest.mark.gpu
 @pytest.mark.parametrize("block", [0, 32, 96, 512])
-def test_specialized_rnea_block_sizes_and_ragged_tail(block, monkeypatch):
+def test_specialized_block_sizes_and_ragged_tail(block, monkeypatch):
     """Any block size (a run-time value) and a batch that ends in the middle of a warp."""
     monkeypatch.setenv("BARD_SPEC_MIN_B", "0")
     if block:
@@ -117,21 +148,40 @@ def test_specialized_rnea_block_sizes_and_ragged_tail(block, monkeypatch):
     desc = W.config_robot(3)
     s = Spec(desc)
     q, qd, qdd = W.config_states(3, 5000 + 13)
-    ref = s.o.rnea(*(a.astype(np.float64) for a in (q, qd, qdd)))
-    assert nerr(s.rnea(q, qd, qdd), ref) <= TOL_DYN
+    s.check(s.run(q, qd, qdd), s.refs(q, qd, qdd))
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("cfg,B", [(3, 65536), (1, 65536), (0, 1048576)])
-def test_specialized_rnea_full_size_sampled(cfg, B):
+def test_specialized_jacobian_follows_set_frames(monkeypatch):
+    monkeypatch.setenv("BARD_SPEC_MIN_B", "0")
+    desc = W.config_robot(3)
+    s = Spec(desc)
+    q, qd, qdd = W.config_states(3, 257)
+    s.check(s.run(q, qd, qdd), s.refs(q, qd, qdd))
+    desc.frame_body = [5, 23, 14]                                  # new frames: team kernel until specialised again
+    desc.frame_offset = [[0.1, 0.0, -0.2], [0.0, 0.0, 0.0], [0.0, 0.3, 0.0]]
+    s.m.set_frames(desc.frame_body, desc.frame_offset)
+    s.o = oracle.Oracle(desc)
+    s.check(s.run(q, qd, qdd), s.refs(q, qd, qdd))
+    s.m.specialize(("jacobian",))
+    assert "frame 2 on body 14" in s.m.specialized_source("jacobian")
+    s.check(s.run(q, qd, qdd), s.refs(q, qd, qdd))
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("cfg,B", [(3, 65536), (1, 65536), (2, 65536), (0, 1048576)])
+def test_specialized_full_size_sampled(cfg, B):
     """bench.py's launch configuration (default knobs): a strided sample of environments against the oracle."""
     desc = W.config_robot(cfg)
     s = Spec(desc)
     q, qd, qdd = W.config_states(cfg, B)
-    tau = s.rnea(q, qd, qdd)
-    assert np.isfinite(tau).all()
+    out = s.run(q, qd, qdd)
     idx = np.unique(np.concatenate([np.arange(0, B, max(1, B // 997)), [B - 1, B - 2, 127, 128, B // 2]]))
-    ref = s.o.rnea(*(np.ascontiguousarray(a[:, idx].astype(np.float64)) for a in (q, qd, qdd)))
-    assert nerr(tau[:, idx], ref) <= TOL_DYN
-    again = s.rnea(q, qd, qdd)
-    assert np.array_equal(tau, again)                              # no atomics, fixed child order
+    ref = s.refs(*(a[:, idx] for a in (q, qd, qdd)))
+    for a in out:
+        assert np.isfinite(a).all()
+    for a, r, tol in zip(out, ref, (TOL_KIN, TOL_KIN, TOL_DYN, TOL_DYN)):
+        assert nerr(a[..., idx], r) <= tol
+    again = s.run(q, qd, qdd)
+    for a, b in zip(out, again):
+        assert np.array_equal(a, b)                                # no atomics, fixed child order
