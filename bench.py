@@ -302,16 +302,30 @@ def run_ours(args):
     # ---- device-resident timed region: W warm-up steps, then exactly K steps
     for i in range(Wm):
         step(i)
-    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(K)]
+    # The timed region is K uninstrumented steps between two events: an event record between two launches would
+    # end the programmatic overlap of a kernel's prologue with the previous kernel's tail (PDL) and time the
+    # events themselves.  Per-operator durations come from a second, identical pass of K steps with an event
+    # before every launch (below); its step time is reported next to the headline as ms_per_step_instrumented.
+    e_beg, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     clocks.active.set()
     n0 = binding.launch_count()
+    e_beg.record()
+    for i in range(K):
+        step(i)
+    e_end.record()
+    barrier()
+    clocks.active.clear()
+    launches = binding.launch_count() - n0
+    elapsed_ms = e_beg.elapsed_time(e_end)
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(K)]
+    barrier()
+    clocks.active.set()
     for i in range(K):
         step(i, evs[i])
     barrier()
     clocks.active.clear()
-    launches = binding.launch_count() - n0
-    elapsed_ms = evs[0][0].elapsed_time(evs[-1][4])
+    instrumented_ms = evs[0][0].elapsed_time(evs[-1][4])
     t = torch.tensor([elapsed_ms], device=dev, dtype=torch.float64)
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -381,12 +395,14 @@ def run_ours(args):
 
     dom = max(OPS, key=lambda o: op_sec[o])
     d = ops[dom]
-    roof = {"kernel": f"{dom}_kernel", "bound": d["bound"], "achieved": d["achieved"], "peak": d["peak"],
+    spec = (not args.no_specialize) and dom in SPEC_OPS
+    roof = {"kernel": f"bard_{dom}_n1 (model-specialised)" if spec else f"{dom}_kernel", "bound": d["bound"], "achieved": d["achieved"], "peak": d["peak"],
             "unit": d["unit"], "frac": d["frac"], "traffic": None,
             "peak_source": ("MEASURED_PEAKS.json hbm_gbs" if d["bound"] == "hbm" else
                             "derived: 148 SM x 128 lanes x 2 x sm_max_mhz") + f" ({pk['source']})",
             "algorithmic_per_launch": (d["bytes_per_env"] if d["bound"] == "hbm" else d["flop_per_env"]) * B,
-            "avg_launch_us": d["us"]}
+            "avg_launch_us": d["us"],
+            "timing": "CUDA events before every launch, second pass of K steps identical to the timed region"}
     tr = os.path.join(ROOT, "profiles", "traffic.json")   # dram bytes per launch from the committed ncu capture
     if os.path.exists(tr):
         try:
@@ -396,7 +412,7 @@ def run_ours(args):
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
-        "ms_per_step": elapsed_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": elapsed_ms / K, "ms_per_step_instrumented": instrumented_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": workload_name(cfg, B), "envs_per_gpu": B, "global_envs": world * B,
                    "parallelism": f"batch-sharded x{world}, no collective",
