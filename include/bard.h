@@ -105,10 +105,12 @@ bard_status bard_model_get_table(const bard_model* m, int table_id, void* host_d
 bard_status bard_model_set_frames(bard_model* m, int32_t nframes, const int32_t* body, const double* offset);
 
 /* Operators, as bits of the `ops` mask of bard_model_specialize. */
-enum { BARD_OP_FK = 1, BARD_OP_JACOBIAN = 2, BARD_OP_RNEA = 4, BARD_OP_CRBA = 8 };
+enum { BARD_OP_FK = 1, BARD_OP_JACOBIAN = 2, BARD_OP_RNEA = 4, BARD_OP_CRBA = 8,
+       BARD_OP_STEP = 15,     /* all four, each as its own kernel                                   */
+       BARD_OP_FUSED = 16 };  /* the fused kernel behind bard_step                                  */
 
 /* Model-specialised kernels (optional, once per model, takes seconds): writes straight-line CUDA source of
- * the operators in `ops` for THIS model -- constants as literals, the tree walked depth first so that the
+ * the operators in `ops` (BARD_OP_FUSED: one kernel that evaluates all four, see bard_step) for THIS model -- constants as literals, the tree walked depth first so that the
  * inward pass of a subtree follows its outward pass (eq. (6)) and only the bodies on
  * the current root-to-leaf path hold parked state -- compiles it for sm_100a with NVRTC (libnvrtc.so.12 of the
  * CUDA toolkit, loaded with dlopen) and loads the cubin.  Afterwards bard_<op> calls with a large batch
@@ -132,6 +134,14 @@ bard_status bard_rnea(const bard_model* m, int64_t B, const float* q, const floa
                       float* tau, bard_stream stream);
 /* CRBA: composite-inertia backward sweep (the X^T M X update of PAPER.md:103) and mass-matrix fill. */
 bard_status bard_crba(const bard_model* m, int64_t B, const float* q, float* M, bard_stream stream);
+
+/* One simulation step's worth of operators on one batch: poses, Jacobians, torques and mass matrix of the same
+ * (q, qd, qdd) -- the paper's tiered cache and "full pipeline" restated on chip.  If the model
+ * was specialised with BARD_OP_FUSED and the batch is in the specialised regime, ONE kernel evaluates the joint
+ * transforms and FK once per body and shares them between the four operators; otherwise bard_fk, bard_jacobian,
+ * bard_rnea and bard_crba are enqueued in that order on `stream`.  Outputs and layouts as for the four calls. */
+bard_status bard_step(const bard_model* m, int64_t B, const float* q, const float* qd, const float* qdd,
+                      float* pose, float* J, float* tau, float* M, bard_stream stream);
 
 const char* bard_status_string(bard_status s);
 const char* bard_last_error(void);

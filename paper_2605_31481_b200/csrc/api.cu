@@ -118,7 +118,7 @@ static bard_status check_call(const char* fn, const bard_model* bm, int64_t B, c
 bard_status bard_fk(const bard_model* bm, int64_t B, const float* q, float* pose, bard_stream stream) {
   bard_status s = check_call("bard_fk", bm, B, bm && bm->m.nq == 0 ? (const void*)pose : q, pose, pose, pose);
   if (s != BARD_OK || B == 0) return s;
-  if (bard::launch_fk_specialized(bm->m, B, q, pose, stream, s)) return s;
+  if (bard::launch_specialized(bm->m, BARD_OP_FK, B, q, nullptr, nullptr, pose, nullptr, nullptr, nullptr, stream, s)) return s;
   return bard::launch_fk(bm->m, B, q, pose, stream);
 }
 
@@ -126,7 +126,7 @@ bard_status bard_jacobian(const bard_model* bm, int64_t B, const float* q, float
   if (bm && (bm->m.nframes == 0 || bm->m.nv == 0)) return check_call("bard_jacobian", bm, B, bm, bm, bm, bm);  // empty output
   bard_status s = check_call("bard_jacobian", bm, B, bm->m.nq == 0 ? (const void*)J : q, J, J, J);
   if (s != BARD_OK || B == 0) return s;
-  if (bard::launch_jacobian_specialized(bm->m, B, q, J, stream, s)) return s;
+  if (bard::launch_specialized(bm->m, BARD_OP_JACOBIAN, B, q, nullptr, nullptr, nullptr, J, nullptr, nullptr, stream, s)) return s;
   return bard::launch_jacobian(bm->m, B, q, J, stream);
 }
 
@@ -135,7 +135,7 @@ bard_status bard_rnea(const bard_model* bm, int64_t B, const float* q, const flo
   if (bm && bm->m.nv == 0) return check_call("bard_rnea", bm, B, bm, bm, bm, bm);  // nothing to write
   bard_status s = check_call("bard_rnea", bm, B, q, qd, qdd, tau);
   if (s != BARD_OK || B == 0) return s;
-  if (bard::launch_rnea_specialized(bm->m, B, q, qd, qdd, tau, stream, s)) return s;
+  if (bard::launch_specialized(bm->m, BARD_OP_RNEA, B, q, qd, qdd, nullptr, nullptr, tau, nullptr, stream, s)) return s;
   return bard::launch_rnea(bm->m, B, q, qd, qdd, tau, stream);
 }
 
@@ -143,8 +143,26 @@ bard_status bard_crba(const bard_model* bm, int64_t B, const float* q, float* M,
   if (bm && bm->m.nv == 0) return check_call("bard_crba", bm, B, bm, bm, bm, bm);
   bard_status s = check_call("bard_crba", bm, B, q, M, M, M);
   if (s != BARD_OK || B == 0) return s;
-  if (bard::launch_crba_specialized(bm->m, B, q, M, stream, s)) return s;
+  if (bard::launch_specialized(bm->m, BARD_OP_CRBA, B, q, nullptr, nullptr, nullptr, nullptr, nullptr, M, stream, s)) return s;
   return bard::launch_crba(bm->m, B, q, M, stream);
+}
+
+bard_status bard_step(const bard_model* bm, int64_t B, const float* q, const float* qd, const float* qdd, float* pose, float* J,
+                      float* tau, float* M, bard_stream stream) {
+  if (!bm) { set_error("bard_step: model is NULL"); return BARD_ERR_INVALID_ARG; }
+  // the fused kernel needs all four outputs to exist; otherwise (no DOF, no frames, not specialised, small batch)
+  // the step is the four operators in sequence on the same stream
+  if (bm->m.nv > 0 && bm->m.nframes > 0) {
+    bard_status s = check_call("bard_step", bm, B, q, qd, qdd, tau);
+    if (s == BARD_OK) s = check_call("bard_step", bm, B, pose, J, M, M);
+    if (s != BARD_OK || B == 0) return s;
+    if (bard::launch_specialized(bm->m, BARD_OP_STEP, B, q, qd, qdd, pose, J, tau, M, stream, s)) return s;
+  }
+  bard_status s = bard_fk(bm, B, q, pose, stream);
+  if (s == BARD_OK) s = bard_jacobian(bm, B, q, J, stream);
+  if (s == BARD_OK) s = bard_rnea(bm, B, q, qd, qdd, tau, stream);
+  if (s == BARD_OK) s = bard_crba(bm, B, q, M, stream);
+  return s;
 }
 
 const char* bard_status_string(bard_status s) {

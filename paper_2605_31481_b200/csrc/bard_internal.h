@@ -136,11 +136,8 @@ bard_status launch_crba(const Model& m, int64_t B, const float* q, float* M, voi
 bard_status specialize(Model& M, uint32_t ops);
 void free_specialized(Specialized* s);
 const std::string* specialized_source(const Model& M, uint32_t op);
-bool launch_rnea_specialized(const Model& M, int64_t B, const float* q, const float* qd, const float* qdd, float* tau,
-                             void* stream, bard_status& st);
-bool launch_fk_specialized(const Model& M, int64_t B, const float* q, float* pose, void* stream, bard_status& st);
-bool launch_jacobian_specialized(const Model& M, int64_t B, const float* q, float* J, void* stream, bard_status& st);
+bool launch_specialized(const Model& M, uint32_t op, int64_t B, const float* q, const float* qd, const float* qdd, float* pose,
+                        float* J, float* tau, float* Mo, void* stream, bard_status& st);
 void drop_specialized_jacobian(Model& M);
-bool launch_crba_specialized(const Model& M, int64_t B, const float* q, float* Mo, void* stream, bard_status& st);
 
 }  // namespace bard

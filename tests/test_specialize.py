@@ -31,9 +31,11 @@ def test_generated_source_compiles_on_host(idx):
     """A host-only model: the source is generated and NVRTC-compiled for sm_100a, nothing is loaded."""
     desc = _robots()[idx]
     m = binding.Model(desc, device=-1)
-    m.specialize(ALL)
+    m.specialize(ALL + ("fused",))
     for op in ALL:
         assert 'extern "C" __global__' in m.specialized_source(op) and f"bard_{op}_n1" in m.specialized_source(op)
+    if m.nv > 0 and m.nframes > 0:
+        assert "bard_step_n1" in m.specialized_source("fused")
     # FK: 12 rows per body; CRBA / Jacobian: every output row stored exactly once (fill + structural zeros)
     for op, arr, n in (("fk", "pose", 12 * m.nb), ("crba", "Mo", m.nv * m.nv), ("jacobian", "J", 6 * m.nframes * m.nv)):
         rows = sorted(int(r) for r in re.findall(r"strow\(%s, (\d+)u \* B \+ e" % arr, m.specialized_source(op)))
@@ -149,6 +151,50 @@ def test_specialized_block_sizes_and_ragged_tail(block, monkeypatch):
     s = Spec(desc)
     q, qd, qdd = W.config_states(3, 5000 + 13)
     s.check(s.run(q, qd, qdd), s.refs(q, qd, qdd))
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("idx", [0, 1, 2, 4, 5, 7, 9])
+def test_fused_step_matches_oracle_and_the_four_calls(idx, monkeypatch):
+    """bard_step: one fused kernel where it is built (small parked state), else the four operators; both against
+    the oracle, and the fused outputs against the four specialised kernels bit for bit (same generated arithmetic)."""
+    monkeypatch.setenv("BARD_SPEC_MIN_B", "0")
+    monkeypatch.setenv("BARD_SPEC_FUSED_MAX_ROWS", "100000")      # build the fused kernel for every robot here
+    desc = _robots()[idx]
+    s = Spec(desc)
+    s.m.specialize(("fused",))
+    q, qd, qdd = W.sample_states(desc, 700, seed=40 + idx)
+    four = s.run(q, qd, qdd)
+    m, B, dev = s.m, 700, s.dev
+    tq, tqd, tqdd = (torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in (q, qd, qdd))
+    outs = [torch.full(sh, float("nan"), device=dev) for sh in ((m.nb, 12, B), (m.nframes, 6, m.nv, B), (m.nv, B), (m.nv, m.nv, B))]
+    n0 = binding.launch_count()
+    m.step(B, tq, tqd, tqdd, *outs, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert binding.launch_count() - n0 == (1 if m.nv > 0 and m.nframes > 0 else 4) or m.nv == 0
+    fused = [t.cpu().numpy() for t in outs]
+    s.check(fused, s.refs(q, qd, qdd))
+    for a, b in zip(fused, four):
+        assert nerr(a, b.astype(np.float64)) <= 1e-5
+
+
+@pytest.mark.gpu
+def test_step_without_specialisation_is_the_four_team_kernels():
+    desc = W.config_robot(1)
+    m = binding.Model(desc, device=0)
+    o = oracle.Oracle(desc)
+    B = 300
+    q, qd, qdd = W.config_states(1, B)
+    dev = torch.device("cuda:0")
+    tq, tqd, tqdd = (torch.from_numpy(a).to(dev) for a in (q, qd, qdd))
+    outs = [torch.full(sh, float("nan"), device=dev) for sh in ((m.nb, 12, B), (m.nframes, 6, m.nv, B), (m.nv, B), (m.nv, m.nv, B))]
+    n0 = binding.launch_count()
+    m.step(B, tq, tqd, tqdd, *outs, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert binding.launch_count() - n0 == 4
+    q64, qd64, qdd64 = (a.astype(np.float64) for a in (q, qd, qdd))
+    for t, r, tol in zip(outs, (o.fk(q64), o.jacobian(q64), o.rnea(q64, qd64, qdd64), o.crba(q64)), (TOL_KIN, TOL_KIN, TOL_DYN, TOL_DYN)):
+        assert nerr(t.cpu().numpy(), r) <= tol
 
 
 @pytest.mark.gpu
