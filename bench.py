@@ -49,6 +49,7 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--sweep", action="store_true", help="also time every operator over config 4's batch sweep")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-rollout", action="store_true", help="skip the config-2 24-step rollout section")
     ap.add_argument("--no-specialize", action="store_true",
                     help="skip bard_model_specialize: every operator runs its table-driven team kernel")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU work for the oracle baseline")
@@ -247,6 +248,59 @@ def time_op_graph(torch, m, op, sets, B, launches=64, replays=10):
     return e0.elapsed_time(e1) * 1e-3 / (launches * replays)
 
 
+def rollout_config2(torch, binding, dev, specialize=True, steps=24, dt=0.005, replays=10):
+    """BASELINE.json config 2: the 11-DOF spined quadruped, all four operators per simulated RL step (bard_step)
+    over 24 consecutive steps, q advanced on the device by explicit Euler (bard_euler_step) from seeded random qdd.
+    The 24-step loop is captured once into a CUDA graph and replayed; reported as env-steps/s."""
+    desc = W.config_robot(2)
+    m = binding.Model(desc, device=dev.index or 0)
+    if specialize:
+        m.specialize(SPEC_OPS)
+    out = {}
+    for B in (4096, 65536):
+        q, qd, _ = W.sample_states(desc, B, seed=2002)
+        q0, qd0 = torch.from_numpy(q).to(dev), torch.from_numpy(qd).to(dev)
+        tq, tqd = q0.clone(), qd0.clone()
+        qdds = [torch.from_numpy(np.random.default_rng(2002 + 100 * (k + 1)).normal(size=(desc.nv, B)).astype(np.float32)).to(dev)
+                for k in range(steps)]
+        outs = [torch.empty(sh, device=dev) for sh in ((m.nb, 12, B), (m.nframes, 6, m.nv, B), (m.nv, B), (m.nv, m.nv, B))]
+
+        def loop(stream):
+            for k in range(steps):
+                m.step(B, tq, tqd, qdds[k], *outs, stream)
+                m.euler_step(B, dt, tq, tqd, qdds[k], stream)
+
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            loop(side.cuda_stream)                       # warm-up (also loads every kernel before capture)
+        torch.cuda.current_stream().wait_stream(side)
+        torch.cuda.synchronize()
+        n0 = binding.launch_count()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            loop(side.cuda_stream)
+        per_loop = binding.launch_count() - n0
+        tq.copy_(q0); tqd.copy_(qd0)
+        g.replay()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ms = []
+        for _ in range(replays):
+            tq.copy_(q0); tqd.copy_(qd0)                 # every replay integrates the same 24 steps
+            e0.record()
+            g.replay()
+            e1.record()
+            torch.cuda.synchronize()
+            ms.append(e0.elapsed_time(e1))
+        med = float(np.median(ms))
+        out[f"B{B}"] = {"env_steps_per_s": B * steps / (med * 1e-3), "us_per_step": med * 1e3 / steps,
+                        "ms_per_24_steps": med, "launches_per_24_steps": int(per_loop), "finite": bool(torch.isfinite(outs[3]).all())}
+    m.close()
+    out["note"] = "CUDA graph of 24 x (bard_step + bard_euler_step), dt 0.005, seeded qdd per step, median of 10 replays"
+    return out
+
+
 def op_report(desc, pk, op, sec, B):
     r = RL.roofline(desc, pk)[op]
     if r["bound"] == "hbm":
@@ -427,6 +481,11 @@ def run_ours(args):
     }
     if args.sweep and rank == 0:
         line["sweep"] = sweep(torch, binding, pk, dev, stream, specialize=not args.no_specialize)
+    if rank == 0 and world == 1 and not args.no_rollout:
+        try:
+            line["config2_rollout"] = rollout_config2(torch, binding, dev, specialize=not args.no_specialize)
+        except Exception as ex:                          # graph capture is a convenience of the bench, not of the path
+            line["config2_rollout"] = {"error": str(ex)[:200]}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cb, _, _ = time_oracle(desc, cfg, args.cpu_seconds)
         line["cpu_baseline"] = cb

@@ -143,6 +143,14 @@ bard_status bard_crba(const bard_model* m, int64_t B, const float* q, float* M, 
 bard_status bard_step(const bard_model* m, int64_t B, const float* q, const float* qd, const float* qdd,
                       float* pose, float* J, float* tau, float* M, bard_stream stream);
 
+/* Explicit Euler step on the configuration manifold, IN PLACE (BASELINE.json config 2: "q advanced by explicit
+ * Euler from random qdd"; the paper's RL loop calls the operators once per simulated step):
+ *   qd += dt qdd ;  q (+)= dt qd
+ * revolute / prismatic: q += dt qd; free joint (q = [p, quat xyzw], qd = body-frame twist [v; omega]):
+ * p += dt R(quat) v, quat += dt/2 quat (x) (omega, 0), renormalised.  One kernel launch, asynchronous. */
+bard_status bard_euler_step(const bard_model* m, int64_t B, float dt, float* q, float* qd, const float* qdd,
+                            bard_stream stream);
+
 const char* bard_status_string(bard_status s);
 const char* bard_last_error(void);
 /* Number of kernel launches this process has enqueued through the library (bench.py's gpu_launches). */

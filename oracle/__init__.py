@@ -71,6 +71,7 @@ def lib():
         L.bard_oracle_rnea.argtypes = [P, C.c_int64, dp, dp, dp, dp]
         L.bard_oracle_crba.argtypes = [P, C.c_int64, dp, dp]
         L.bard_oracle_body_velocity.argtypes = [P, C.c_int64, dp, dp, dp]
+        L.bard_oracle_euler_step.argtypes = [P, C.c_int64, C.c_double, dp, dp, dp]
         L.bard_oracle_spatial_inertia.argtypes = [P, C.c_int32, dp]
         L.bard_oracle_set_threads.argtypes = [C.c_int]
         L.bard_oracle_get_threads.restype = C.c_int
@@ -210,6 +211,14 @@ class Oracle:
         out = np.zeros((self.nv, self.nv, B))
         self._chk(lib().bard_oracle_crba(C.byref(self._d), B, _dptr(q), _dptr(out)))
         return out
+
+    def euler_step(self, dt, q, qd, qdd):
+        """One explicit Euler step of the config-2 rollout: returns the new (q, qd)."""
+        q = np.array(self._in(q, self.nq), copy=True)
+        qd = np.array(self._in(qd, self.nv), copy=True)
+        qdd = self._in(qdd, self.nv)
+        self._chk(lib().bard_oracle_euler_step(C.byref(self._d), q.shape[1], float(dt), _dptr(q), _dptr(qd), _dptr(qdd)))
+        return q, qd
 
     def body_velocity(self, q, qd) -> np.ndarray:
         q = self._in(q, self.nq)

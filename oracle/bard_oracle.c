@@ -608,6 +608,42 @@ int bard_oracle_body_velocity(const bard_oracle_desc* d, int64_t B, const double
   return 0;
 }
 
+/* Explicit Euler step of config 2 (BASELINE.json; readings 1 and 15), in place:
+ *   qd += dt qdd ; q (+)= dt qd
+ * revolute / prismatic: q += dt qd.  Free joint (q = [p, quat xyzw], qd = body-frame twist [v; omega]):
+ *   p += dt R(quat) v ;  quat += dt/2 quat (x) (omega, 0) ;  quat /= |quat|      (quat normalised first)
+ * The rotation is taken from joint_T, the same routine FK uses. */
+int bard_oracle_euler_step(const bard_oracle_desc* d, int64_t B, double dt, double* q, double* qd, const double* qdd) {
+  omodel* m = (omodel*)malloc(sizeof(omodel));
+  int rc = build_model(d, m);
+  if (rc) { free(m); return rc; }
+  for (int64_t b = 0; b < B; ++b) {
+    for (int j = 0; j < m->nv; ++j) qd[(int64_t)j * B + b] += dt * qdd[(int64_t)j * B + b];
+    for (int i = 0; i < m->nb; ++i) {
+      const int t = m->jtype[i], qo = m->qoff[i], vo = m->voff[i];
+      if (t == JT_REVOLUTE || t == JT_PRISMATIC) {
+        q[(int64_t)qo * B + b] += dt * qd[(int64_t)vo * B + b];
+      } else if (t == JT_FREE) {
+        double qi[7], TJ[16], v[3], w[3];
+        gather_q(m, i, q, B, b, qi);
+        joint_T(m, i, qi, TJ);
+        for (int k = 0; k < 3; ++k) { v[k] = qd[(int64_t)(vo + k) * B + b]; w[k] = qd[(int64_t)(vo + 3 + k) * B + b]; }
+        for (int r = 0; r < 3; ++r)
+          q[(int64_t)(qo + r) * B + b] = qi[r] + dt * (TJ[r * 4] * v[0] + TJ[r * 4 + 1] * v[1] + TJ[r * 4 + 2] * v[2]);
+        double n = sqrt(qi[3] * qi[3] + qi[4] * qi[4] + qi[5] * qi[5] + qi[6] * qi[6]);
+        double x = qi[3] / n, y = qi[4] / n, z = qi[5] / n, s = qi[6] / n;
+        /* Hamilton product (x, y, z; s) (x) (w; 0) */
+        double e[4] = {x + 0.5 * dt * (s * w[0] + y * w[2] - z * w[1]), y + 0.5 * dt * (s * w[1] + z * w[0] - x * w[2]),
+                       z + 0.5 * dt * (s * w[2] + x * w[1] - y * w[0]), s + 0.5 * dt * (-x * w[0] - y * w[1] - z * w[2])};
+        n = sqrt(e[0] * e[0] + e[1] * e[1] + e[2] * e[2] + e[3] * e[3]);
+        for (int k = 0; k < 4; ++k) q[(int64_t)(qo + 3 + k) * B + b] = e[k] / n;
+      }
+    }
+  }
+  free(m);
+  return 0;
+}
+
 int bard_oracle_spatial_inertia(const bard_oracle_desc* d, int32_t body, double* I66) {
   omodel* m = (omodel*)malloc(sizeof(omodel));
   int rc = build_model(d, m);

@@ -83,6 +83,10 @@ int  bard_oracle_rnea    (const bard_oracle_desc* d, int64_t B, const double* q,
                           const double* qdd, double* tau);
 int  bard_oracle_crba    (const bard_oracle_desc* d, int64_t B, const double* q, double* M);
 
+/* explicit Euler step of the config-2 rollout, in place: qd += dt qdd ; q (+)= dt qd (manifold step for a
+ * free joint: p += dt R v, quat += dt/2 quat (x) (omega, 0), renormalised) */
+int  bard_oracle_euler_step(const bard_oracle_desc* d, int64_t B, double dt, double* q, double* qd, const double* qdd);
+
 /* spatial velocity of every body, body coordinates, API order [lin; ang]: vel[nb][6][B]
  * (used by the invariants: kinetic energy, frame velocity = J qd) */
 int  bard_oracle_body_velocity(const bard_oracle_desc* d, int64_t B, const double* q,

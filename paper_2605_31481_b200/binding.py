@@ -25,7 +25,7 @@ TABLES = {"LEVEL_PTR": (0, np.int32), "LEVEL_BODY": (1, np.int32), "BODY_LEVEL":
           "PARENT_SLOT": (3, np.int32), "Q_OFF": (4, np.int32), "V_OFF": (5, np.int32), "DOF_BODY": (6, np.int32),
           "ANC_MASK": (7, np.uint64), "RODRIGUES": (8, np.float32)}
 EXPORTS = ["bard_model_create", "bard_model_destroy", "bard_model_dims", "bard_model_get_table",
-           "bard_model_set_frames", "bard_model_specialize", "bard_model_specialized_source", "bard_fk", "bard_jacobian", "bard_rnea", "bard_crba", "bard_step",
+           "bard_model_set_frames", "bard_model_specialize", "bard_model_specialized_source", "bard_fk", "bard_jacobian", "bard_rnea", "bard_crba", "bard_step", "bard_euler_step",
            "bard_status_string", "bard_last_error", "bard_launch_count"]
 
 
@@ -67,6 +67,7 @@ def lib():
         L.bard_rnea.argtypes = [vp, i64, fp, fp, fp, fp, vp]
         L.bard_crba.argtypes = [vp, i64, fp, fp, vp]
         L.bard_step.argtypes = [vp, i64, fp, fp, fp, fp, fp, fp, fp, vp]
+        L.bard_euler_step.argtypes = [vp, i64, C.c_float, fp, fp, fp, vp]
         L.bard_status_string.argtypes = [C.c_int]
         L.bard_status_string.restype = C.c_char_p
         L.bard_last_error.restype = C.c_char_p
@@ -191,6 +192,10 @@ class Model:
         """All four operators of one (q, qd, qdd) batch: one fused kernel if specialised with "fused"."""
         _check(lib().bard_step(self._h, int(B), _ptr(q), _ptr(qd), _ptr(qdd), _ptr(pose), _ptr(J), _ptr(tau), _ptr(M),
                                stream or None))
+
+    def euler_step(self, B, dt, q, qd, qdd, stream=0):
+        """qd += dt qdd ; q (+)= dt qd in place (``bard_euler_step``)."""
+        _check(lib().bard_euler_step(self._h, int(B), float(dt), _ptr(q), _ptr(qd), _ptr(qdd), stream or None))
 
     def crba(self, B, q, M, stream=0):
         _check(lib().bard_crba(self._h, int(B), _ptr(q), _ptr(M), stream or None))

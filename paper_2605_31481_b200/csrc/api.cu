@@ -165,6 +165,13 @@ bard_status bard_step(const bard_model* bm, int64_t B, const float* q, const flo
   return s;
 }
 
+bard_status bard_euler_step(const bard_model* bm, int64_t B, float dt, float* q, float* qd, const float* qdd, bard_stream stream) {
+  if (bm && bm->m.nq == 0) return check_call("bard_euler_step", bm, B, bm, bm, bm, bm);   // nothing to integrate
+  bard_status s = check_call("bard_euler_step", bm, B, q, bm->m.nv ? (const void*)qd : q, bm->m.nv ? (const void*)qdd : q, q);
+  if (s != BARD_OK || B == 0) return s;
+  return bard::launch_euler(bm->m, B, dt, q, qd, qdd, stream);
+}
+
 const char* bard_status_string(bard_status s) {
   switch (s) {
     case BARD_OK: return "BARD_OK";
