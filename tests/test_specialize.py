@@ -179,6 +179,31 @@ def test_fused_step_matches_oracle_and_the_four_calls(idx, monkeypatch):
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("cfg,B", [(3, 1000), (2, 777), (3, 65536)])
+def test_side_by_side_step_is_one_launch_and_bit_equal_to_the_four_kernels(cfg, B, monkeypatch):
+    """Where the fused kernel does not pay, bard_step is ONE launch of the four specialised operators side by side
+    (blockIdx.y = operator): the same generated code, so the same bits as the four separate launches."""
+    monkeypatch.setenv("BARD_SPEC_MIN_B", "0")
+    monkeypatch.setenv("BARD_SPEC_FUSED_MAX_ROWS", "0")           # never the fused kernel ...
+    monkeypatch.setenv("BARD_SPEC_FUSED_SMALL_B", "0")            # ... at any batch size
+    monkeypatch.setenv("BARD_SPEC_STEP4_MAX_ROWS", "100000")      # build the side-by-side kernel for every robot here
+    desc = W.config_robot(cfg)
+    s = Spec(desc)
+    s.m.specialize(("fused",))
+    q, qd, qdd = W.config_states(cfg, B)
+    four = s.run(q, qd, qdd)
+    m, dev = s.m, s.dev
+    tq, tqd, tqdd = (torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in (q, qd, qdd))
+    outs = [torch.full(sh, float("nan"), device=dev) for sh in ((m.nb, 12, B), (m.nframes, 6, m.nv, B), (m.nv, B), (m.nv, m.nv, B))]
+    n0 = binding.launch_count()
+    m.step(B, tq, tqd, tqdd, *outs, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert binding.launch_count() - n0 == 1
+    for t, ref in zip(outs, four):
+        assert np.array_equal(t.cpu().numpy(), ref)
+
+
+@pytest.mark.gpu
 def test_step_without_specialisation_is_the_four_team_kernels():
     desc = W.config_robot(1)
     m = binding.Model(desc, device=0)
