@@ -414,6 +414,22 @@ def run_ours(args):
                 small[op]["cuda_graph"] = {k: rg[k] for k in ("us", "env_evals_per_s", "frac")}
             except Exception as ex:                      # graph capture is a convenience of the bench, not of the path
                 small[op]["cuda_graph"] = {"error": str(ex)[:120]}
+        # the whole step at B = 4096 through bard_step (fused kernel, or the four operators forked over side streams)
+        def steps_4096(n):
+            for i in range(n):
+                x = sets_s[i % len(sets_s)]
+                m.step(4096, x.q, x.qd, x.qdd, x.pose, x.J, x.tau, x.M, stream)
+        steps_4096(10)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        n0 = binding.launch_count()
+        e0.record()
+        steps_4096(200)
+        e1.record()
+        barrier()
+        us = e0.elapsed_time(e1) * 1e3 / 200
+        small["step"] = {"us": us, "env_evals_per_s": 4096 / (us * 1e-6), "launches_per_step": (binding.launch_count() - n0) / 200,
+                         "sum_of_operator_trains_us": sum(small[op]["us"] for op in OPS)}
         del sets_s
     clocks.active.clear()
 

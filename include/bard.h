@@ -139,7 +139,10 @@ bard_status bard_crba(const bard_model* m, int64_t B, const float* q, float* M, 
  * (q, qd, qdd) -- the paper's tiered cache and "full pipeline" restated on chip.  If the model
  * was specialised with BARD_OP_FUSED and the batch is in the specialised regime, ONE kernel evaluates the joint
  * transforms and FK once per body and shares them between the four operators; otherwise bard_fk, bard_jacobian,
- * bard_rnea and bard_crba are enqueued in that order on `stream`.  Outputs and layouts as for the four calls. */
+ * bard_rnea and bard_crba are enqueued on `stream` -- for small batches (B <= 16384, where one operator's grid does
+ * not fill the machine) forked over three internal side streams and joined back into `stream`, so the step costs
+ * its longest operator, not the sum; the fork-join is ordered after everything already in `stream`, is complete
+ * before anything enqueued later, and can be captured into a CUDA graph.  Outputs and layouts as for the four calls. */
 bard_status bard_step(const bard_model* m, int64_t B, const float* q, const float* qd, const float* qdd,
                       float* pose, float* J, float* tau, float* M, bard_stream stream);
 

@@ -2,13 +2,25 @@
 #include <cuda_runtime.h>
 
 #include <atomic>
+#include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "bard_internal.h"
 
+// bard_step's fork-join: three side streams and the events that order them against the caller's stream.
+// Created once with the model, so that bard_step itself allocates nothing.
+struct StepFork {
+  cudaStream_t side[3] = {nullptr, nullptr, nullptr};
+  cudaEvent_t fork = nullptr, join[3] = {nullptr, nullptr, nullptr};
+  std::mutex mu;              // one fork-join is enqueued at a time (the events are re-recorded by every call)
+  bool ok = false;
+};
+
 struct bard_model {
   bard::Model m;
+  StepFork fj;
 };
 
 namespace bard {
@@ -29,6 +41,19 @@ bard_status bard_model_create(const bard_model_desc* desc, int cuda_device, bard
   if (!bm) { set_error("bard_model_create: host allocation failed"); return BARD_ERR_ALLOC; }
   bard_status s = bard::build_model(desc, cuda_device, bm->m);
   if (s != BARD_OK) { delete bm; return s; }
+  if (bm->m.d_blob) {         // device model: the fork-join plumbing of bard_step (not fatal if it cannot be created)
+    int prev = 0;
+    cudaGetDevice(&prev);
+    cudaSetDevice(bm->m.device);
+    StepFork& f = bm->fj;
+    bool ok = cudaEventCreateWithFlags(&f.fork, cudaEventDisableTiming) == cudaSuccess;
+    for (int k = 0; k < 3 && ok; ++k)
+      ok = cudaStreamCreateWithFlags(&f.side[k], cudaStreamNonBlocking) == cudaSuccess &&
+           cudaEventCreateWithFlags(&f.join[k], cudaEventDisableTiming) == cudaSuccess;
+    f.ok = ok;
+    if (!ok) cudaGetLastError();
+    cudaSetDevice(prev);
+  }
   *out = bm;
   return BARD_OK;
 }
@@ -41,6 +66,11 @@ void bard_model_destroy(bard_model* bm) {
     cudaSetDevice(bm->m.device);
     cudaFree(bm->m.d_blob);
     if (bm->m.d_jblob) cudaFree(bm->m.d_jblob);
+    for (int k = 0; k < 3; ++k) {
+      if (bm->fj.side[k]) cudaStreamDestroy(bm->fj.side[k]);
+      if (bm->fj.join[k]) cudaEventDestroy(bm->fj.join[k]);
+    }
+    if (bm->fj.fork) cudaEventDestroy(bm->fj.fork);
     cudaSetDevice(prev);
   }
   bard::free_specialized(bm->m.spec);
@@ -157,6 +187,28 @@ bard_status bard_step(const bard_model* bm, int64_t B, const float* q, const flo
     if (s == BARD_OK) s = check_call("bard_step", bm, B, pose, J, M, M);
     if (s != BARD_OK || B == 0) return s;
     if (bard::launch_specialized(bm->m, BARD_OP_STEP, B, q, qd, qdd, pose, J, tau, M, stream, s)) return s;
+  }
+  // Small batches: one operator's grid does not fill the machine (B = 4096: 128 tiles on 148 SMs), and the four
+  // operators are independent given (q, qd, qdd) -- fork them over three side streams and join, so the step costs
+  // its longest operator instead of the sum.  Works under stream capture (the side streams join the capture).
+  static const int64_t fork_max_b = [] { const char* v = std::getenv("BARD_STEP_FORK_MAX_B"); return v ? std::atoll(v) : 16384ll; }();
+  StepFork& f = const_cast<bard_model*>(bm)->fj;
+  if (f.ok && B > 0 && B <= fork_max_b && bm->m.nv > 0) {
+    std::lock_guard<std::mutex> lock(f.mu);
+    cudaStream_t user = (cudaStream_t)stream;
+    bool ok = cudaEventRecord(f.fork, user) == cudaSuccess;
+    for (int k = 0; k < 3 && ok; ++k) ok = cudaStreamWaitEvent(f.side[k], f.fork, 0) == cudaSuccess;
+    if (ok) {
+      bard_status s = bard_crba(bm, B, q, M, stream);           // the longest operator stays on the caller's stream
+      bard_status s1 = bard_jacobian(bm, B, q, J, f.side[0]);
+      bard_status s2 = bard_rnea(bm, B, q, qd, qdd, tau, f.side[1]);
+      bard_status s3 = bard_fk(bm, B, q, pose, f.side[2]);
+      for (int k = 0; k < 3; ++k)                               // always join, whatever the launches returned
+        if (cudaEventRecord(f.join[k], f.side[k]) != cudaSuccess || cudaStreamWaitEvent(user, f.join[k], 0) != cudaSuccess) ok = false;
+      if (!ok) { set_error(std::string("bard_step: fork-join: ") + cudaGetErrorString(cudaGetLastError())); return BARD_ERR_CUDA; }
+      return s != BARD_OK ? s : s1 != BARD_OK ? s1 : s2 != BARD_OK ? s2 : s3;
+    }
+    cudaGetLastError();                                         // could not fork: fall through to the plain sequence
   }
   bard_status s = bard_fk(bm, B, q, pose, stream);
   if (s == BARD_OK) s = bard_jacobian(bm, B, q, J, stream);

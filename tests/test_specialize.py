@@ -223,6 +223,25 @@ def test_step_without_specialisation_is_the_four_team_kernels():
 
 
 @pytest.mark.gpu
+def test_specialized_max_size_tree_and_single_fixed_body(monkeypatch):
+    """The compiled limits (64 bodies, 16 frames) and the degenerate model (one fixed body: no q, no DOF)."""
+    monkeypatch.setenv("BARD_SPEC_MIN_B", "0")
+    desc = W.random_tree(4242, nb=64, shape="random", nframes=16)
+    s = Spec(desc)
+    q, qd, qdd = W.sample_states(desc, 96, seed=5)
+    s.check(s.run(q, qd, qdd), s.refs(q, qd, qdd))
+    one = W.build_robot("one_fixed", [-1], [W.FIXED], seed=1)
+    m = binding.Model(one, device=0)
+    m.specialize(ALL + ("fused",))
+    pose = torch.full((1, 12, 8), float("nan"), device="cuda:0")
+    n0 = binding.launch_count()
+    m.fk(8, None, pose, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert binding.launch_count() - n0 == 1
+    assert nerr(pose.cpu().numpy(), oracle.Oracle(one).fk(np.zeros((0, 8)))) <= TOL_KIN
+
+
+@pytest.mark.gpu
 def test_specialized_jacobian_follows_set_frames(monkeypatch):
     monkeypatch.setenv("BARD_SPEC_MIN_B", "0")
     desc = W.config_robot(3)
