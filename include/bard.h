@@ -107,7 +107,8 @@ bard_status bard_model_set_frames(bard_model* m, int32_t nframes, const int32_t*
 /* Operators, as bits of the `ops` mask of bard_model_specialize. */
 enum { BARD_OP_FK = 1, BARD_OP_JACOBIAN = 2, BARD_OP_RNEA = 4, BARD_OP_CRBA = 8,
        BARD_OP_STEP = 15,     /* all four, each as its own kernel                                   */
-       BARD_OP_FUSED = 16 };  /* the fused kernel behind bard_step                                  */
+       BARD_OP_FUSED = 16,    /* the fused kernel behind bard_step                                  */
+       BARD_OP_ABA = 32 };    /* forward dynamics (bard_aba): exists only as a specialised kernel   */
 
 /* Model-specialised kernels (optional, once per model, takes seconds): writes straight-line CUDA source of
  * the operators in `ops` (BARD_OP_FUSED: one kernel that evaluates all four, see bard_step) for THIS model -- constants as literals, the tree walked depth first so that the
@@ -153,6 +154,17 @@ bard_status bard_step(const bard_model* m, int64_t B, const float* q, const floa
  * p += dt R(quat) v, quat += dt/2 quat (x) (omega, 0), renormalised.  One kernel launch, asynchronous. */
 bard_status bard_euler_step(const bard_model* m, int64_t B, float dt, float* q, float* qd, const float* qdd,
                             bard_stream stream);
+
+/* ABA forward dynamics, the paper's fifth operator: qdd = M(q)^-1 (tau - C(q, qd)) by the
+ * articulated-body algorithm -- three passes, the 6x6 update I^A_parent += X^T I^a X of PAPER.md:103 on the way up.
+ * tau[nv][B] in, qdd[nv][B] out (free joint: [linear; angular] blocks as everywhere), gravity as in bard_rnea.
+ * Needs bard_model_specialize(model, BARD_OP_ABA) first (there is no table-driven ABA kernel: BARD_ERR_UNSUPPORTED
+ * otherwise, also for a free joint that is not on a root body) and a caller-owned device workspace of
+ * bard_aba_workspace_floats(model, B) floats (10 nv B: what the downward acceleration pass needs of every body).
+ * One launch, asynchronous. */
+size_t      bard_aba_workspace_floats(const bard_model* m, int64_t B);
+bard_status bard_aba(const bard_model* m, int64_t B, const float* q, const float* qd, const float* tau, float* qdd,
+                     float* workspace, bard_stream stream);
 
 const char* bard_status_string(bard_status s);
 const char* bard_last_error(void);

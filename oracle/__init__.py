@@ -220,6 +220,18 @@ class Oracle:
         self._chk(lib().bard_oracle_euler_step(C.byref(self._d), q.shape[1], float(dt), _dptr(q), _dptr(qd), _dptr(qdd)))
         return q, qd
 
+    def aba(self, q, qd, tau) -> np.ndarray:
+        """Forward dynamics by its definition: the qdd that solves M(q) qdd + C(q, qd) = tau, with M from CRBA,
+        C = RNEA(q, qd, 0) (gravity included) and a dense fp64 solve per environment (numpy.linalg.solve).  The
+        paper's ABA reaches exactly this result by an O(n) recursion."""
+        q = self._in(q, self.nq)
+        qd = self._in(qd, self.nv)
+        tau = self._in(tau, self.nv)
+        M = self.crba(q)                                      # [nv, nv, B]
+        C0 = self.rnea(q, qd, np.zeros_like(qd))              # [nv, B]
+        rhs = (tau - C0).T[:, :, None]                        # [B, nv, 1]
+        return np.ascontiguousarray(np.linalg.solve(np.moveaxis(M, 2, 0), rhs)[:, :, 0].T)
+
     def body_velocity(self, q, qd) -> np.ndarray:
         q = self._in(q, self.nq)
         qd = self._in(qd, self.nv)

@@ -20,12 +20,12 @@ from . import build as _build
 BARD_OK = 0
 STATUS = {0: "BARD_OK", 1: "BARD_ERR_INVALID_ARG", 2: "BARD_ERR_TOPOLOGY", 3: "BARD_ERR_UNSUPPORTED",
           4: "BARD_ERR_ALLOC", 5: "BARD_ERR_CUDA"}
-OPS = {"fk": 1, "jacobian": 2, "rnea": 4, "crba": 8, "fused": 16}
+OPS = {"fk": 1, "jacobian": 2, "rnea": 4, "crba": 8, "fused": 16, "aba": 32}
 TABLES = {"LEVEL_PTR": (0, np.int32), "LEVEL_BODY": (1, np.int32), "BODY_LEVEL": (2, np.int32),
           "PARENT_SLOT": (3, np.int32), "Q_OFF": (4, np.int32), "V_OFF": (5, np.int32), "DOF_BODY": (6, np.int32),
           "ANC_MASK": (7, np.uint64), "RODRIGUES": (8, np.float32)}
 EXPORTS = ["bard_model_create", "bard_model_destroy", "bard_model_dims", "bard_model_get_table",
-           "bard_model_set_frames", "bard_model_specialize", "bard_model_specialized_source", "bard_fk", "bard_jacobian", "bard_rnea", "bard_crba", "bard_step", "bard_euler_step",
+           "bard_model_set_frames", "bard_model_specialize", "bard_model_specialized_source", "bard_fk", "bard_jacobian", "bard_rnea", "bard_crba", "bard_step", "bard_euler_step", "bard_aba", "bard_aba_workspace_floats",
            "bard_status_string", "bard_last_error", "bard_launch_count"]
 
 
@@ -68,6 +68,9 @@ def lib():
         L.bard_crba.argtypes = [vp, i64, fp, fp, vp]
         L.bard_step.argtypes = [vp, i64, fp, fp, fp, fp, fp, fp, fp, vp]
         L.bard_euler_step.argtypes = [vp, i64, C.c_float, fp, fp, fp, vp]
+        L.bard_aba.argtypes = [vp, i64, fp, fp, fp, fp, fp, vp]
+        L.bard_aba_workspace_floats.argtypes = [vp, i64]
+        L.bard_aba_workspace_floats.restype = C.c_size_t
         L.bard_status_string.argtypes = [C.c_int]
         L.bard_status_string.restype = C.c_char_p
         L.bard_last_error.restype = C.c_char_p
@@ -196,6 +199,13 @@ class Model:
     def euler_step(self, B, dt, q, qd, qdd, stream=0):
         """qd += dt qdd ; q (+)= dt qd in place (``bard_euler_step``)."""
         _check(lib().bard_euler_step(self._h, int(B), float(dt), _ptr(q), _ptr(qd), _ptr(qdd), stream or None))
+
+    def aba_workspace_floats(self, B) -> int:
+        return int(lib().bard_aba_workspace_floats(self._h, int(B)))
+
+    def aba(self, B, q, qd, tau, qdd, workspace, stream=0):
+        """Forward dynamics qdd = M^-1 (tau - C) (``bard_aba``); needs ``specialize(("aba",))`` first."""
+        _check(lib().bard_aba(self._h, int(B), _ptr(q), _ptr(qd), _ptr(tau), _ptr(qdd), _ptr(workspace), stream or None))
 
     def crba(self, B, q, M, stream=0):
         _check(lib().bard_crba(self._h, int(B), _ptr(q), _ptr(M), stream or None))

@@ -224,6 +224,19 @@ bard_status bard_euler_step(const bard_model* bm, int64_t B, float dt, float* q,
   return bard::launch_euler(bm->m, B, dt, q, qd, qdd, stream);
 }
 
+size_t bard_aba_workspace_floats(const bard_model* bm, int64_t B) {
+  return (bm && B > 0) ? (size_t)10 * (size_t)bm->m.nv * (size_t)B : 0;
+}
+
+bard_status bard_aba(const bard_model* bm, int64_t B, const float* q, const float* qd, const float* tau, float* qdd, float* workspace,
+                     bard_stream stream) {
+  if (bm && bm->m.nv == 0) return check_call("bard_aba", bm, B, bm, bm, bm, bm);  // nothing to write
+  bard_status s = check_call("bard_aba", bm, B, q, qd, tau, qdd);
+  if (s == BARD_OK && B > 0 && !workspace) { set_error("bard_aba: workspace is NULL"); s = BARD_ERR_INVALID_ARG; }
+  if (s != BARD_OK || B == 0) return s;
+  return bard::launch_aba(bm->m, B, q, qd, tau, qdd, workspace, stream);
+}
+
 const char* bard_status_string(bard_status s) {
   switch (s) {
     case BARD_OK: return "BARD_OK";

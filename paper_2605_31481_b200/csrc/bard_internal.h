@@ -140,5 +140,6 @@ const std::string* specialized_source(const Model& M, uint32_t op);
 bool launch_specialized(const Model& M, uint32_t op, int64_t B, const float* q, const float* qd, const float* qdd, float* pose,
                         float* J, float* tau, float* Mo, void* stream, bard_status& st);
 void drop_specialized_jacobian(Model& M);
+bard_status launch_aba(const Model& M, int64_t B, const float* q, const float* qd, const float* tau, float* qdd, float* ws, void* stream);
 
 }  // namespace bard

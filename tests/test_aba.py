@@ -1,0 +1,164 @@
+"""ABA forward dynamics (the paper's fifth operator).
+Oracle = the definition: solve M(q) qdd = tau - C(q, qd) in fp64; pinned by closed forms and the RNEA round trip.
+GPU = the generated three-pass articulated-body kernel (bard_aba); parity on the forward error and on the residual."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2605_31481_b200 import binding, workloads as W
+
+TOL = 1e-3        # north_star's tolerance for dynamics quantities (tau, M); qdd inherits it (reading 19)
+EPS32 = 2.0 ** -24
+
+
+def aba_checks(o, q64, qd64, tau64, qdd_gpu):
+    """Forward error against the oracle and componentwise backward error of M qdd + C = tau.
+    Forward: per element |qdd - ref| / max(1, |ref|) <= max(1e-3, 4 eps32 cond(M)) -- solving with M amplifies fp32
+    rounding by its condition number (the paper's own ABA row is 1e5 x its RNEA row in fp64);
+    on the BASELINE robots cond(M) <= 1e4 and the bound is the plain 1e-3.
+    Backward: |RNEA(q, qd, qdd) - tau|_i <= 1e-3 max(1, |tau_i|, sum_j |M_ij| |qdd_j|)."""
+    ref = o.aba(q64, qd64, tau64)
+    M = o.crba(q64)
+    cond = max(np.linalg.cond(M[:, :, b]) for b in range(0, M.shape[2], max(1, M.shape[2] // 16)))
+    fwd = nerr(qdd_gpu, ref)
+    assert fwd <= max(TOL, 4 * EPS32 * cond), (fwd, cond)
+    h = qdd_gpu.astype(np.float64)
+    res = np.abs(o.rnea(q64, qd64, h) - tau64)
+    scale = np.maximum(1.0, np.maximum(np.abs(tau64), np.einsum("ijb,jb->ib", np.abs(M), np.abs(h))))
+    assert float((res / scale).max()) <= TOL
+
+
+def nerr(x, ref):
+    return float(np.max(np.abs(x.astype(np.float64) - ref) / np.maximum(1.0, np.abs(ref)))) if ref.size else 0.0
+
+
+# ------------------------------------------------------------------------------------------- oracle pins (CPU)
+def _pendulum(m=1.3, l=0.7, Iyy=0.05):
+    T = np.zeros((1, 12)); T[0, [0, 5, 10]] = 1.0
+    return W.RobotDesc(name="pendulum", parent=np.array([-1], np.int32), joint_type=np.array([W.REVOLUTE], np.int32),
+                       axis=np.array([[0.0, 1.0, 0.0]]), T_pre=T, T_post=None, mass=np.array([m]),
+                       com=np.array([[0.0, 0.0, -l]]), inertia=np.array([[0.02, 0, 0, Iyy, 0, 0.03]]),
+                       gravity=np.array([0.0, 0.0, -9.81]))
+
+
+def test_oracle_aba_single_pendulum_closed_form():
+    """(I_yy + m l^2) qdd + m g l sin q = tau  (SURVEY 8(c) pins: single pendulum)."""
+    m, l, Iyy = 1.3, 0.7, 0.05
+    o = oracle.Oracle(_pendulum(m, l, Iyy))
+    rng = np.random.default_rng(1)
+    q, qd, tau = rng.uniform(-3, 3, (1, 50)), rng.normal(size=(1, 50)), rng.normal(size=(1, 50))
+    ref = (tau - m * 9.81 * l * np.sin(q)) / (Iyy + m * l * l)
+    assert np.abs(o.aba(q, qd, tau) - ref).max() <= 1e-12
+
+
+def test_oracle_aba_free_body_newton_euler():
+    """Single free body: the spatial equation [F; N] = I a + v x* I v solved for the acceleration in closed form
+    (COM at the origin here, so linear and angular parts decouple): v_dot = F/m - w x v + R^T g, w_dot = I^-1 (N - w x I w)."""
+    desc = W.build_robot("free1", [-1], [W.FREE], seed=3)
+    desc.com[:] = 0.0
+    o = oracle.Oracle(desc)
+    q, qd, tau = W.sample_states(desc, 40, seed=9, dtype=np.float64)
+    qdd = o.aba(q, qd, tau)
+    m = desc.mass[0]
+    Ic = desc.inertia[0]
+    I3 = np.array([[Ic[0], Ic[1], Ic[2]], [Ic[1], Ic[3], Ic[4]], [Ic[2], Ic[4], Ic[5]]])
+    from scipy.spatial.transform import Rotation
+    R = Rotation.from_quat(q[3:7].T).as_matrix()                       # [B,3,3]
+    v, w = qd[0:3].T, qd[3:6].T
+    g = np.asarray(desc.gravity)
+    vdot = tau[0:3].T / m - np.cross(w, v) + np.einsum("bji,j->bi", R, g)
+    wdot = np.linalg.solve(I3, (tau[3:6].T - np.cross(w, w @ I3.T)).T).T
+    assert np.abs(qdd[0:3].T - vdot).max() <= 1e-10
+    assert np.abs(qdd[3:6].T - wdot).max() <= 1e-10
+
+
+@pytest.mark.parametrize("idx", range(6))
+def test_oracle_aba_round_trip_through_rnea(idx):
+    """RNEA(q, qd, ABA(q, qd, tau)) = tau on the BASELINE robots and random trees (RNEA is pinned on its own)."""
+    desc = ([W.config_robot(c) for c in range(4)] + [W.random_tree(31, 12, free_root=True), W.random_tree(32, 20)])[idx]
+    o = oracle.Oracle(desc)
+    q, qd, tau = W.sample_states(desc, 32, seed=50 + idx, dtype=np.float64)
+    qdd = o.aba(q, qd, tau)
+    assert np.abs(o.rnea(q, qd, qdd) - tau).max() <= 1e-8 * max(1.0, np.abs(qdd).max())
+
+
+def test_aba_needs_specialisation_and_compiles_on_host():
+    m = binding.Model(W.config_robot(1), device=-1)
+    m.specialize(("aba",))
+    src = m.specialized_source("aba")
+    assert "bard_aba_n1" in src and src.count("(accelerations)") == m.nb
+    assert m.aba_workspace_floats(1000) == 10 * m.nv * 1000
+    # a free joint below another body: refused
+    bad = W.build_robot("free_child", [-1, 0], [W.REVOLUTE, W.FREE], seed=2)
+    mb = binding.Model(bad, device=-1)
+    with pytest.raises(binding.BardError) as e:
+        mb.specialize(("aba",))
+    assert e.value.code == 3
+
+
+# ------------------------------------------------------------------------------------------- GPU
+torch = pytest.importorskip("torch")
+
+
+def _robots():
+    out = [W.config_robot(c) for c in range(4)]
+    for seed in range(6):
+        shape = ["random", "chain", "star", "unbalanced"][seed % 4]
+        out.append(W.random_tree(800 + seed, nb=2 + 4 * seed, shape=shape, free_root=(seed % 2 == 0)))
+    return out
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("idx", range(10))
+@pytest.mark.parametrize("B", [1, 130, 1000 + 7])
+def test_gpu_aba_matches_oracle(idx, B):
+    desc = _robots()[idx]
+    m = binding.Model(desc, device=0)
+    m.specialize(("aba",))
+    o = oracle.Oracle(desc)
+    dev = torch.device("cuda:0")
+    q, qd, tau = W.sample_states(desc, B, seed=300 + idx)
+    tq, tqd, tt = (torch.from_numpy(a).to(dev) for a in (q, qd, tau))
+    out = torch.full((m.nv, B), float("nan"), device=dev)
+    ws = torch.full((m.aba_workspace_floats(B),), float("nan"), device=dev)
+    n0 = binding.launch_count()
+    m.aba(B, tq, tqd, tt, out, ws, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert binding.launch_count() - n0 == (1 if m.nv else 0)
+    h = out.cpu().numpy()
+    assert np.isfinite(h).all()
+    aba_checks(o, *(a.astype(np.float64) for a in (q, qd, tau)), h)
+    again = torch.full((m.nv, B), float("nan"), device=dev)
+    m.aba(B, tq, tqd, tt, again, ws, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert torch.equal(out, again)
+
+
+@pytest.mark.gpu
+def test_gpu_aba_without_specialisation_is_refused():
+    m = binding.Model(W.config_robot(0), device=0)
+    t = torch.zeros(7, 8, device="cuda:0")
+    with pytest.raises(binding.BardError) as e:
+        m.aba(8, t, t, t, t, t)
+    assert e.value.code == 3
+
+
+@pytest.mark.gpu
+def test_gpu_aba_full_size_sampled():
+    desc = W.config_robot(3)
+    B = 65536
+    m = binding.Model(desc, device=0)
+    m.specialize(("aba",))
+    o = oracle.Oracle(desc)
+    dev = torch.device("cuda:0")
+    q, qd, tau = W.config_states(3, B)
+    tq, tqd, tt = (torch.from_numpy(a).to(dev) for a in (q, qd, tau))
+    out = torch.full((m.nv, B), float("nan"), device=dev)
+    ws = torch.empty(m.aba_workspace_floats(B), device=dev)
+    m.aba(B, tq, tqd, tt, out, ws, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    h = out.cpu().numpy()
+    assert np.isfinite(h).all()
+    idx = np.unique(np.concatenate([np.arange(0, B, B // 499), [B - 1, 447, 448]]))
+    ref = o.aba(*(np.ascontiguousarray(a[:, idx].astype(np.float64)) for a in (q, qd, tau)))
+    assert nerr(h[:, idx], ref) <= TOL
