@@ -497,6 +497,32 @@ def run_ours(args):
     }
     if args.sweep and rank == 0:
         line["sweep"] = sweep(torch, binding, pk, dev, stream, specialize=not args.no_specialize)
+    if rank == 0 and world == 1 and not args.no_specialize and not args.no_rollout and m.nv > 0:
+        # SURVEY 8(f)2, beyond the four operators of the metric: ABA forward dynamics on the same workload (train timing)
+        try:
+            m.specialize(("aba",))
+            ws = torch.empty(m.aba_workspace_floats(B), device=dev)
+            qdd_out = torch.empty((m.nv, B), device=dev)
+
+            def aba_train(n):
+                for i in range(n):
+                    x = sets[i % R]
+                    m.aba(B, x.q, x.qd, x.tau, qdd_out, ws, stream)      # tau of the previous operators as the input torque
+            aba_train(5)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            aba_train(50)
+            e1.record()
+            torch.cuda.synchronize()
+            us = e0.elapsed_time(e1) * 1e3 / 50
+            io = 4 * (m.nq + 3 * m.nv)
+            line["aba"] = {"us": us, "env_evals_per_s": B / (us * 1e-6), "io_bytes_per_env": io, "workspace_bytes_per_env": 40 * m.nv,
+                           "hbm_gbs_io_plus_workspace": (io + 80 * m.nv) * B / (us * 1e-6) / 1e9,
+                           "note": "generated three-pass articulated-body kernel; not part of the headline metric"}
+            del ws, qdd_out
+        except Exception as ex:
+            line["aba"] = {"error": str(ex)[:200]}
     if rank == 0 and world == 1 and not args.no_rollout:
         try:
             line["config2_rollout"] = rollout_config2(torch, binding, dev, specialize=not args.no_specialize)
