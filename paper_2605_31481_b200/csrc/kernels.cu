@@ -50,8 +50,8 @@ struct f2 {
   __device__ __forceinline__ f2() {}
   __device__ __forceinline__ f2(float x, float y) { asm("mov.b64 %0, {%1, %2};" : "=l"(v) : "f"(x), "f"(y)); }
   __device__ __forceinline__ f2(float s) : f2(s, s) {}
-  __device__ __forceinline__ float lo() const { float x, y; asm("mov.b64 {%0, %1}, %2;" : "=f"(x), "=f"(y) : "l"(v)); return x; }
-  __device__ __forceinline__ float hi() const { float x, y; asm("mov.b64 {%0, %1}, %2;" : "=f"(x), "=f"(y) : "l"(v)); return y; }
+  __device__ __forceinline__ float lo() const { return __uint_as_float((unsigned)(v & 0xffffffffull)); }
+  __device__ __forceinline__ float hi() const { return __uint_as_float((unsigned)(v >> 32)); }
 };
 __device__ __forceinline__ f2 operator-(f2 x) { return {-x.lo(), -x.hi()}; }     // folds into an operand modifier
 __device__ __forceinline__ f2 operator+(f2 x, f2 y) { f2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(x.v), "l"(y.v)); return r; }
