@@ -108,7 +108,8 @@ bard_status bard_model_set_frames(bard_model* m, int32_t nframes, const int32_t*
 enum { BARD_OP_FK = 1, BARD_OP_JACOBIAN = 2, BARD_OP_RNEA = 4, BARD_OP_CRBA = 8,
        BARD_OP_STEP = 15,     /* all four, each as its own kernel                                   */
        BARD_OP_FUSED = 16,    /* the fused kernel behind bard_step                                  */
-       BARD_OP_ABA = 32 };    /* forward dynamics (bard_aba): exists only as a specialised kernel   */
+       BARD_OP_ABA = 32,      /* forward dynamics (bard_aba): exists only as a specialised kernel   */
+       BARD_OP_RNEA_ROLES = 64 }; /* bard_model_specialized_source only: the limb-role RNEA kernel  */
 
 /* Model-specialised kernels (optional, once per model, takes seconds): writes straight-line CUDA source of
  * the operators in `ops` (BARD_OP_FUSED: one kernel that evaluates all four, see bard_step) for THIS model -- constants as literals, the tree walked depth first so that the
@@ -116,7 +117,10 @@ enum { BARD_OP_FK = 1, BARD_OP_JACOBIAN = 2, BARD_OP_RNEA = 4, BARD_OP_CRBA = 8,
  * the current root-to-leaf path hold parked state -- compiles it for sm_100a with NVRTC (libnvrtc.so.12 of the
  * CUDA toolkit, loaded with dlopen) and loads the cubin.  Afterwards bard_<op> calls with a large batch
  * launch the specialised kernel (chains: any B; teams of <= 4 warps: B >= 4096; wider: B >= 32768), smaller ones
- * the level-parallel team kernel; results agree to rounding.  The Jacobian is generated for the frames the
+ * the level-parallel team kernel; results agree to rounding.  BARD_OP_RNEA on a single-rooted tree that branches
+ * also builds a limb-role RNEA kernel (the subtrees below the first branching body dealt to two groups of warps
+ * of the CTA, siblings' forces summed in ascending child order through shared memory: PAPER.md:91), which
+ * bard_rnea launches for B <= 256 x SM count, below the thresholds above too.  The Jacobian is generated for the frames the
  * model has at the time of the call: bard_model_set_frames drops it (specialise again afterwards).  Unknown
  * bits: BARD_ERR_INVALID_ARG.  On a host-only model the source is generated and compiled but not loaded.  NVRTC missing or a compile error:
  * BARD_ERR_CUDA with the log in bard_last_error; the model stays usable.  Not thread-safe against concurrent

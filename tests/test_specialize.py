@@ -80,15 +80,39 @@ def test_unknown_operator_bits_are_refused_and_set_frames_drops_the_jacobian():
     assert "frame 0 on body 2" in m.specialized_source("jacobian")
 
 
+def _single_root_and_branches(desc):
+    parent = [int(p) for p in desc.parent]
+    nchild = [parent.count(i) for i in range(len(parent))]
+    return parent.count(-1) == 1 and any(n >= 2 for n in nchild)
+
+
+def test_limb_role_source_on_a_host_only_model(monkeypatch):
+    """The limb-role RNEA kernel is generated where a single-rooted tree branches, one `if (role == r)` stretch per
+    role, forces handed over through park_to and one named barrier; never for a chain."""
+    for roles in (2, 3):
+        monkeypatch.setenv("BARD_SPEC_ROLES", str(roles))
+        m = binding.Model(W.config_robot(3), device=-1)
+        m.specialize(("rnea",))
+        src = m.specialized_source("rnea_roles")
+        for r in range(roles):
+            assert f"if (role == {r}u)" in src
+        assert f"if (role == {roles}u)" not in src
+        assert "park_to<T, N, R>(le," in src and "bar.sync 15" in src and "bar.arrive 15" in src
+    m = binding.Model(W.config_robot(0), device=-1)
+    m.specialize(("rnea",))
+    with pytest.raises(binding.BardError):
+        m.specialized_source("rnea_roles")
+
+
 # ------------------------------------------------------------------------------------------- GPU
 torch = pytest.importorskip("torch")
 
 
 class Spec:
-    def __init__(self, desc):
+    def __init__(self, desc, ops=ALL):
         assert torch.cuda.is_available(), "GPU tests need CUDA; there is no CPU fallback"
         self.m = binding.Model(desc, device=0)
-        self.m.specialize(ALL)
+        self.m.specialize(ops)
         self.o = oracle.Oracle(desc)
         self.dev = torch.device("cuda:0")
 
@@ -132,7 +156,11 @@ def test_specialized_operators_match_oracle(idx, B, monkeypatch):
     s = Spec(desc)
     q, qd, qdd = W.sample_states(desc, B, seed=900 + idx)
     out = s.run(q, qd, qdd)
-    s.check(out, s.refs(q, qd, qdd))
+    ref = s.refs(q, qd, qdd)
+    s.check(out, ref)                                             # RNEA here: limb roles where the tree branches
+    monkeypatch.setenv("BARD_SPEC_ROLES_MAX_B", "0")              # RNEA: one thread per environment
+    out = s.run(q, qd, qdd)
+    s.check(out, ref)
     # and the team kernels on the same inputs: same arithmetic up to the folded zeros
     monkeypatch.setenv("BARD_SPEC_MIN_B", str(1 << 30))
     team = s.run(q, qd, qdd)
@@ -142,15 +170,55 @@ def test_specialized_operators_match_oracle(idx, B, monkeypatch):
 
 @pytest.mark.gpu
 @pytest.mark.parametrize("block", [0, 32, 96, 512])
-def test_specialized_block_sizes_and_ragged_tail(block, monkeypatch):
-    """Any block size (a run-time value) and a batch that ends in the middle of a warp."""
+@pytest.mark.parametrize("roles_max_b", [None, 0])
+def test_specialized_block_sizes_and_ragged_tail(block, roles_max_b, monkeypatch):
+    """Any block size (a run-time value) and a batch that ends in the middle of a warp; RNEA with limb roles
+    (the default at this batch size) and without."""
     monkeypatch.setenv("BARD_SPEC_MIN_B", "0")
     if block:
         monkeypatch.setenv("BARD_SPEC_BLOCK", str(block))
+    if roles_max_b is not None:
+        monkeypatch.setenv("BARD_SPEC_ROLES_MAX_B", str(roles_max_b))
     desc = W.config_robot(3)
     s = Spec(desc)
     q, qd, qdd = W.config_states(3, 5000 + 13)
     s.check(s.run(q, qd, qdd), s.refs(q, qd, qdd))
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("roles", [2, 3, 4])
+@pytest.mark.parametrize("idx", range(10))
+def test_limb_role_rnea_matches_oracle(roles, idx, monkeypatch):
+    """RNEA with the subtrees below the first branching body dealt to `roles` groups of warps: against the oracle,
+    below the specialised regime too (its own rule), and it never runs above its batch limit."""
+    monkeypatch.setenv("BARD_SPEC_ROLES", str(roles))             # read when the kernel is generated
+    monkeypatch.setenv("BARD_SPEC_MIN_B", str(1 << 30))           # roles have their own regime
+    desc = _robots()[idx]
+    s = Spec(desc, ops=("rnea",))
+    dev = torch.device("cuda:0")
+    try:
+        branching = "role == 1u" in s.m.specialized_source("rnea_roles")
+    except binding.BardError:
+        branching = False                                         # a chain or a forest: no limb-role kernel
+    assert branching == _single_root_and_branches(desc)
+    for B in (1, 45, 700):
+        q, qd, qdd = W.sample_states(desc, B, seed=1700 + idx)
+        tq, tqd, tqdd = (torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in (q, qd, qdd))
+        ref = s.o.rnea(*(np.ascontiguousarray(a.astype(np.float64)) for a in (q, qd, qdd)))
+        got = {}
+        for mx in (None, 0):
+            if mx is None:
+                monkeypatch.delenv("BARD_SPEC_ROLES_MAX_B", raising=False)
+            else:
+                monkeypatch.setenv("BARD_SPEC_ROLES_MAX_B", str(mx))
+            tau = torch.full((s.m.nv, B), float("nan"), device=dev)
+            s.m.rnea(B, tq, tqd, tqdd, tau, torch.cuda.current_stream().cuda_stream)
+            torch.cuda.synchronize()
+            got[mx] = tau.cpu().numpy()
+            assert np.isfinite(got[mx]).all()
+            assert nerr(got[mx], ref) <= TOL_DYN
+        if not branching:                                         # a chain: both calls ran the team kernel
+            assert np.array_equal(got[None], got[0])
 
 
 @pytest.mark.gpu
