@@ -104,6 +104,22 @@ def test_limb_role_source_on_a_host_only_model(monkeypatch):
         m.specialized_source("rnea_roles")
 
 
+def test_rnea_source_has_a_variant_without_l2_prefetch(monkeypatch):
+    """RNEA is generated twice by default: with the up-front L2 prefetch (grids of one wave) and without it
+    (`_np`, larger grids); BARD_SPEC_L2PF = 1 / 0 generate one kernel; the other operators always one."""
+    m = binding.Model(W.config_robot(1), device=-1)
+    m.specialize(("rnea", "fk"))
+    src = m.specialized_source("rnea")
+    assert "bard_rnea_n1_np(" in src and "bard_rnea_n1(" in src and "if (PF) {" in src
+    assert "_np(" not in m.specialized_source("fk")
+    for v in ("0", "1"):
+        monkeypatch.setenv("BARD_SPEC_L2PF", v)
+        m = binding.Model(W.config_robot(1), device=-1)
+        m.specialize(("rnea",))
+        src = m.specialized_source("rnea")
+        assert "_np(" not in src and ("pf_l2(q" in src) == (v == "1")
+
+
 # ------------------------------------------------------------------------------------------- GPU
 torch = pytest.importorskip("torch")
 
@@ -343,3 +359,28 @@ def test_specialized_full_size_sampled(cfg, B):
     again = s.run(q, qd, qdd)
     for a, b in zip(out, again):
         assert np.array_equal(a, b)                                # no atomics, fixed child order
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("cfg", [1, 3])
+def test_rnea_variant_without_l2_prefetch_matches(cfg, monkeypatch):
+    """Grids beyond two CTAs per SM run the RNEA variant without the L2 prefetch (here forced with 32-thread CTAs):
+    same arithmetic, so bit-identical to the prefetching variant, and within tolerance of the oracle."""
+    monkeypatch.setenv("BARD_SPEC_MIN_B", "0")
+    monkeypatch.setenv("BARD_SPEC_ROLES_MAX_B", "0")
+    desc = W.config_robot(cfg)
+    s = Spec(desc, ops=("rnea",))
+    B = 32 * 2 * 148 + 32 * 40 + 7                                 # > 2 x SMs CTAs of 32 threads, ragged tail
+    q, qd, qdd = W.sample_states(desc, B, seed=4242 + cfg)
+    o = s.o
+    ref = o.rnea(q.astype(np.float64), qd.astype(np.float64), qdd.astype(np.float64))
+    tq, tqd, tqdd = (torch.from_numpy(np.ascontiguousarray(a)).to(s.dev) for a in (q, qd, qdd))
+    taus = []
+    for block in ("32", "512"):                                    # 337 CTAs (no prefetch) / 22 CTAs (prefetch)
+        monkeypatch.setenv("BARD_SPEC_BLOCK", block)
+        tau = torch.full((s.m.nv, B), float("nan"), device=s.dev)
+        s.m.rnea(B, tq, tqd, tqdd, tau, torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        taus.append(tau.cpu().numpy())
+        assert nerr(taus[-1], ref) <= TOL_DYN
+    assert np.array_equal(taus[0], taus[1])
