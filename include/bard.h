@@ -109,7 +109,8 @@ enum { BARD_OP_FK = 1, BARD_OP_JACOBIAN = 2, BARD_OP_RNEA = 4, BARD_OP_CRBA = 8,
        BARD_OP_STEP = 15,     /* all four, each as its own kernel                                   */
        BARD_OP_FUSED = 16,    /* the fused kernel behind bard_step                                  */
        BARD_OP_ABA = 32,      /* forward dynamics (bard_aba): exists only as a specialised kernel   */
-       BARD_OP_RNEA_ROLES = 64 }; /* bard_model_specialized_source only: the limb-role RNEA kernel  */
+       BARD_OP_RNEA_ROLES = 64,   /* bard_model_specialized_source only: the limb-role RNEA kernel  */
+       BARD_OP_CRBA_ROLES = 128 }; /* bard_model_specialized_source only: the limb-role CRBA kernel */
 
 /* Model-specialised kernels (optional, once per model, takes seconds): writes straight-line CUDA source of
  * the operators in `ops` (BARD_OP_FUSED: one kernel that evaluates all four, see bard_step) for THIS model -- constants as literals, the tree walked depth first so that the

@@ -20,7 +20,7 @@ from . import build as _build
 BARD_OK = 0
 STATUS = {0: "BARD_OK", 1: "BARD_ERR_INVALID_ARG", 2: "BARD_ERR_TOPOLOGY", 3: "BARD_ERR_UNSUPPORTED",
           4: "BARD_ERR_ALLOC", 5: "BARD_ERR_CUDA"}
-OPS = {"fk": 1, "jacobian": 2, "rnea": 4, "crba": 8, "fused": 16, "aba": 32, "rnea_roles": 64}
+OPS = {"fk": 1, "jacobian": 2, "rnea": 4, "crba": 8, "fused": 16, "aba": 32, "rnea_roles": 64, "crba_roles": 128}
 TABLES = {"LEVEL_PTR": (0, np.int32), "LEVEL_BODY": (1, np.int32), "BODY_LEVEL": (2, np.int32),
           "PARENT_SLOT": (3, np.int32), "Q_OFF": (4, np.int32), "V_OFF": (5, np.int32), "DOF_BODY": (6, np.int32),
           "ANC_MASK": (7, np.uint64), "RODRIGUES": (8, np.float32)}

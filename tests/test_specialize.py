@@ -174,7 +174,8 @@ def test_specialized_operators_match_oracle(idx, B, monkeypatch):
     out = s.run(q, qd, qdd)
     ref = s.refs(q, qd, qdd)
     s.check(out, ref)                                             # RNEA here: limb roles where the tree branches
-    monkeypatch.setenv("BARD_SPEC_ROLES_MAX_B", "0")              # RNEA: one thread per environment
+    monkeypatch.setenv("BARD_SPEC_ROLES_MAX_B", "0")              # RNEA and CRBA: one thread per environment
+    monkeypatch.setenv("BARD_SPEC_CRBA_ROLES_MAX_B", "0")
     out = s.run(q, qd, qdd)
     s.check(out, ref)
     # and the team kernels on the same inputs: same arithmetic up to the folded zeros
@@ -195,6 +196,7 @@ def test_specialized_block_sizes_and_ragged_tail(block, roles_max_b, monkeypatch
         monkeypatch.setenv("BARD_SPEC_BLOCK", str(block))
     if roles_max_b is not None:
         monkeypatch.setenv("BARD_SPEC_ROLES_MAX_B", str(roles_max_b))
+        monkeypatch.setenv("BARD_SPEC_CRBA_ROLES_MAX_B", str(roles_max_b))
     desc = W.config_robot(3)
     s = Spec(desc)
     q, qd, qdd = W.config_states(3, 5000 + 13)
@@ -235,6 +237,43 @@ def test_limb_role_rnea_matches_oracle(roles, idx, monkeypatch):
             assert nerr(got[mx], ref) <= TOL_DYN
         if not branching:                                         # a chain: both calls ran the team kernel
             assert np.array_equal(got[None], got[0])
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("roles", [2, 3])
+@pytest.mark.parametrize("idx", range(10))
+def test_limb_role_crba_matches_oracle(roles, idx, monkeypatch):
+    """CRBA with limb roles (composite inertias of the other roles' subtrees handed over in the world frame, rows of a
+    subtree's DOFs against the trunk filled by the subtree's role): every entry of M written, symmetric bit for bit,
+    against the oracle and against the one-thread-per-environment kernel."""
+    monkeypatch.setenv("BARD_SPEC_ROLES", str(roles))             # read when the kernel is generated
+    monkeypatch.setenv("BARD_SPEC_MIN_B", "0")
+    desc = _robots()[idx]
+    s = Spec(desc, ops=("crba",))
+    dev = torch.device("cuda:0")
+    try:
+        branching = "role == 1u" in s.m.specialized_source("crba_roles")
+    except binding.BardError:
+        branching = False
+    assert branching == _single_root_and_branches(desc)
+    for B in (1, 45, 700):
+        q, _, _ = W.sample_states(desc, B, seed=2700 + idx)
+        tq = torch.from_numpy(np.ascontiguousarray(q)).to(dev)
+        ref = s.o.crba(np.ascontiguousarray(q.astype(np.float64)))
+        got = {}
+        for mx in (1 << 30, 0):
+            monkeypatch.setenv("BARD_SPEC_CRBA_ROLES_MAX_B", str(mx))
+            monkeypatch.setenv("BARD_SPEC_CRBA_ROLES_MIN_B", "0")
+            Mo = torch.full((s.m.nv, s.m.nv, B), float("nan"), device=dev)
+            s.m.crba(B, tq, Mo, torch.cuda.current_stream().cuda_stream)
+            torch.cuda.synchronize()
+            got[mx] = Mo.cpu().numpy()
+            assert np.isfinite(got[mx]).all()
+            assert nerr(got[mx], ref) <= TOL_DYN
+            assert np.array_equal(got[mx], np.swapaxes(got[mx], 0, 1))
+        assert nerr(got[1 << 30], got[0].astype(np.float64)) <= 1e-4
+        if not branching:
+            assert np.array_equal(got[1 << 30], got[0])
 
 
 @pytest.mark.gpu
