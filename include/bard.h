@@ -27,6 +27,11 @@
  *
  * Execution: operator calls enqueue exactly one kernel on `stream`, allocate nothing and never
  * synchronise.  B == 0 returns BARD_OK without a launch.  Outputs are fully overwritten.
+ * Devices: a model lives on the device given to bard_model_create; `stream` and every device pointer of
+ * a call must belong to that device.  The calling thread's current device may be any: every call makes the
+ * model's device current for its duration and restores the caller's.
+ * Threads: operator calls on one model from several host threads / on several streams are legal (the
+ * model is immutable between bard_model_create / set_frames / set_option / specialize calls).
  *
  * Errors: return codes only; bard_last_error() gives thread-local detail text.
  */
@@ -45,7 +50,7 @@ typedef void* bard_stream;                /* a cudaStream_t (NULL = default stre
 
 typedef enum {
   BARD_OK = 0,
-  BARD_ERR_INVALID_ARG = 1,   /* NULL pointer, negative B, nb < 1, bad joint type, zero axis, mass <= 0,
+  BARD_ERR_INVALID_ARG = 1,   /* NULL pointer, negative B, nb < 1, bad joint type, zero axis, mass < 0,
                                  non-identity T_post on a free joint, bad frame body */
   BARD_ERR_TOPOLOGY = 2,      /* parent[i] >= i or < -1 (topological numbering is required) */
   BARD_ERR_UNSUPPORTED = 3,   /* nb > BARD_MAX_BODIES or nv > BARD_MAX_DOF or B too large */
@@ -70,7 +75,7 @@ typedef struct {
                                  ignored for FIXED / FREE                                          */
   const double*  T_pre;       /* [nb*12] rows [R|t]: the paper's T_joint (parent body -> joint)    */
   const double*  T_post;      /* [nb*12] or NULL = identity: the paper's T_link; identity for FREE */
-  const double*  mass;        /* [nb]   > 0                                                        */
+  const double*  mass;        /* [nb]   >= 0 (massless links are legal; bard_aba needs positive inertia under every DOF) */
   const double*  com;         /* [nb*3] body frame                                                 */
   const double*  inertia;     /* [nb*6] xx,xy,xz,yy,yz,zz about the COM, body axes                 */
   double         gravity[3];  /* world frame, e.g. (0,0,-9.81)                                     */
@@ -101,8 +106,22 @@ bard_status bard_model_dims(const bard_model* m, int32_t* nb, int32_t* nq, int32
  * nothing is copied and BARD_ERR_INVALID_ARG is returned (call with cap 0 to query). */
 bard_status bard_model_get_table(const bard_model* m, int table_id, void* host_dst, size_t cap, size_t* need);
 /* Choose the Jacobian frames: frame f is rigidly attached to body[f] at `offset` (body coordinates,
- * [nframes*3], NULL = zeros).  Not thread-safe against concurrent bard_jacobian calls. */
+ * [nframes*3], NULL = zeros).  A build-time call: it SYNCHRONISES the model's device first (the J tables are
+ * rewritten in place and the generated Jacobian / step kernels are unloaded, so no kernel that reads them -- on any
+ * stream, blocking or not, including bard_step's internal side streams -- may still be in flight), then uploads.
+ * Not thread-safe against concurrent operator calls on the same model from other host threads. */
 bard_status bard_model_set_frames(bard_model* m, int32_t nframes, const int32_t* body, const double* offset);
+
+/* Launch / code-generation knobs are fields of the model, never global state: bard_model_create reads the default of
+ * option "x" once from the environment variable BARD_X (upper case), bard_model_set_option overrides it; no operator
+ * call reads the environment.  Keys (int64 values, -1 = the documented automatic rule): teams, pack, pack2_min_b,
+ * pdl (team kernels); spec_min_b, spec_block, spec_roles_max_b, spec_crba_roles_max_b, spec_crba_roles_min_b,
+ * spec_fused_max_rows, spec_fused_small_b, spec_kin_min_b, step_fork_max_b (which kernel a call gets: take effect at
+ * the next operator call); spec_prefetch, spec_sync, spec_l2pf, spec_roles, spec_zero_role, spec_maxreg, spec_step4,
+ * spec_step4_max_rows, spec_pair (code generation: take effect at the next bard_model_specialize).
+ * section 10.  Unknown key: BARD_ERR_INVALID_ARG.  Not thread-safe against concurrent operator calls on the model. */
+bard_status bard_model_set_option(bard_model* m, const char* key, int64_t value);
+bard_status bard_model_get_option(const bard_model* m, const char* key, int64_t* value);
 
 /* Operators, as bits of the `ops` mask of bard_model_specialize. */
 enum { BARD_OP_FK = 1, BARD_OP_JACOBIAN = 2, BARD_OP_RNEA = 4, BARD_OP_CRBA = 8,

@@ -73,6 +73,9 @@ def lib():
         L.bard_oracle_body_velocity.argtypes = [P, C.c_int64, dp, dp, dp]
         L.bard_oracle_euler_step.argtypes = [P, C.c_int64, C.c_double, dp, dp, dp]
         L.bard_oracle_spatial_inertia.argtypes = [P, C.c_int32, dp]
+        L.bard_oracle_rnea_params.argtypes = [P, C.c_int64, dp, dp, dp, dp, dp]
+        L.bard_oracle_inertial_params.argtypes = [P, dp]
+        L.bard_oracle_rnea_vjp_params.argtypes = [P, C.c_int64, dp, dp, dp, dp, dp]
         L.bard_oracle_set_threads.argtypes = [C.c_int]
         L.bard_oracle_get_threads.restype = C.c_int
         _lib = L
@@ -231,6 +234,33 @@ class Oracle:
         C0 = self.rnea(q, qd, np.zeros_like(qd))              # [nv, B]
         rhs = (tau - C0).T[:, :, None]                        # [B, nv, 1]
         return np.ascontiguousarray(np.linalg.solve(np.moveaxis(M, 2, 0), rhs)[:, :, 0].T)
+
+    # -- RNEA as a function of the inertial parameters (SURVEY 8(f)3) --------------------
+    def inertial_params(self) -> np.ndarray:
+        """[nb, 10]: m, h = m c, Io (xx,xy,xz,yy,yz,zz about the body origin) of every link of the description."""
+        out = np.zeros((self.nb, 10))
+        self._chk(lib().bard_oracle_inertial_params(C.byref(self._d), _dptr(out)))
+        return out
+
+    def rnea_params(self, q, qd, qdd, params) -> np.ndarray:
+        q = self._in(q, self.nq)
+        qd = self._in(qd, self.nv)
+        qdd = self._in(qdd, self.nv)
+        params = _f64(params, (self.nb, 10))
+        B = q.shape[1]
+        out = np.zeros((self.nv, B))
+        self._chk(lib().bard_oracle_rnea_params(C.byref(self._d), B, _dptr(q), _dptr(qd), _dptr(qdd), _dptr(params), _dptr(out)))
+        return out
+
+    def rnea_vjp_params(self, q, qd, qdd, dtau) -> np.ndarray:
+        """dparams[nb, 10] = sum_b (d tau_b / d params)^T dtau_b, by the definition (linearity in the parameters)."""
+        q = self._in(q, self.nq)
+        qd = self._in(qd, self.nv)
+        qdd = self._in(qdd, self.nv)
+        dtau = self._in(dtau, self.nv)
+        out = np.zeros((self.nb, 10))
+        self._chk(lib().bard_oracle_rnea_vjp_params(C.byref(self._d), q.shape[1], _dptr(q), _dptr(qd), _dptr(qdd), _dptr(dtau), _dptr(out)))
+        return out
 
     def body_velocity(self, q, qd) -> np.ndarray:
         q = self._in(q, self.nq)

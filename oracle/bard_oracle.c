@@ -724,3 +724,128 @@ int bard_oracle_crba(const bard_oracle_desc* d, int64_t B, const double* q, doub
   free(m);
   return 0;
 }
+
+/* ------------------------------------------------------------------ RNEA as a function of the inertial parameters
+ * the paper's differentiability claim is exercised by identifying link masses through
+ * RNEA (Section 4.3).  tau is LINEAR in the ten inertial parameters of every link,
+ *   theta_i = (m, h = m c (3), Io = Ic + m [c]x [c]x^T : xx, xy, xz, yy, yz, zz about the BODY ORIGIN),
+ * because the spatial inertia I_i = [[Io, [h]x], [[h]x^T, m 1]] is, and f_i = I_i a_i + v_i x* I_i v_i with v, a
+ * independent of theta (RBDA Table 5.1; gravity enters through a_world, so tau(theta = 0) = 0).
+ *
+ * bard_oracle_rnea_params: the recursion of bard_oracle_rnea, line for line, with I_i built from params[nb][10]
+ * instead of (mass, com, inertia).
+ * bard_oracle_rnea_vjp_params: the vector-Jacobian product by its definition,
+ *   dparams[k] = sum_b sum_j dtau[j][b] * d tau[j][b] / d theta_k ,  d tau / d theta_k = tau(theta = e_k)  (linearity),
+ * i.e. nb * 10 evaluations of bard_oracle_rnea_params with unit parameter vectors.  No reverse sweep, no shortcut. */
+static void inertia_from_params(const double* th /* 10 */, double I[36]) {
+  const double m = th[0], h[3] = {th[1], th[2], th[3]};
+  const double Io[9] = {th[4], th[5], th[6], th[5], th[7], th[8], th[6], th[8], th[9]};
+  double hx[9], hxT[9];
+  skew(h, hx);
+  mat_transpose(hx, hxT, 3, 3);
+  for (int r = 0; r < 3; ++r)
+    for (int s = 0; s < 3; ++s) {
+      I[r * 6 + s] = Io[r * 3 + s];
+      I[r * 6 + 3 + s] = hx[r * 3 + s];
+      I[(3 + r) * 6 + s] = hxT[r * 3 + s];
+      I[(3 + r) * 6 + 3 + s] = (r == s) ? m : 0.0;
+    }
+}
+
+static void rnea_with_model(const omodel* m, int64_t B, const double* q, const double* qd, const double* qdd, double* tau) {
+#pragma omp parallel for schedule(static) num_threads(bard_oracle_get_threads())
+  for (int64_t b = 0; b < B; ++b) {
+    double X[MAXB][36], v[MAXB][6], a[MAXB][6], f[MAXB][6];
+    for (int i = 0; i < m->nb; ++i) {
+      double qi[7], Tpc[16], vJ[6], aJ[6], Xv[6], Xa[6], C[36], cv[6];
+      gather_q(m, i, q, B, b, qi);
+      parent_child_T(m, i, qi, Tpc);
+      plucker_X(Tpc, X[i]);
+      joint_velocity(m, i, qd, B, b, vJ);
+      joint_velocity(m, i, qdd, B, b, aJ);
+      int p = m->parent[i];
+      if (p < 0) {
+        for (int k = 0; k < 6; ++k) Xv[k] = 0.0;
+        mat_mul(X[i], m->a_world, Xa, 6, 6, 1);
+      } else {
+        mat_mul(X[i], v[p], Xv, 6, 6, 1);
+        mat_mul(X[i], a[p], Xa, 6, 6, 1);
+      }
+      for (int k = 0; k < 6; ++k) v[i][k] = Xv[k] + vJ[k];
+      crm(v[i], C);
+      mat_mul(C, vJ, cv, 6, 6, 1);
+      for (int k = 0; k < 6; ++k) a[i][k] = Xa[k] + aJ[k] + cv[k];
+      double Ia[6], Iv[6], Cf[36], vIv[6];
+      mat_mul(m->I[i], a[i], Ia, 6, 6, 1);
+      mat_mul(m->I[i], v[i], Iv, 6, 6, 1);
+      crf(v[i], Cf);
+      mat_mul(Cf, Iv, vIv, 6, 6, 1);
+      for (int k = 0; k < 6; ++k) f[i][k] = Ia[k] + vIv[k];
+    }
+    for (int i = m->nb - 1; i >= 0; --i) {
+      int n = m->nvi[i];
+      for (int c = 0; c < n; ++c) {
+        double s = 0.0;
+        for (int r = 0; r < 6; ++r) s += m->S[i][r * n + c] * f[i][r];
+        tau[(int64_t)(m->voff[i] + c) * B + b] = s;
+      }
+      int p = m->parent[i];
+      if (p >= 0) {
+        double XT[36], XTf[6];
+        mat_transpose(X[i], XT, 6, 6);
+        mat_mul(XT, f[i], XTf, 6, 6, 1);
+        for (int k = 0; k < 6; ++k) f[p][k] += XTf[k];
+      }
+    }
+  }
+}
+
+int bard_oracle_rnea_params(const bard_oracle_desc* d, int64_t B, const double* q, const double* qd, const double* qdd,
+                            const double* params, double* tau) {
+  omodel* m = (omodel*)malloc(sizeof(omodel));
+  int rc = build_model(d, m);
+  if (rc) { free(m); return rc; }
+  for (int i = 0; i < m->nb; ++i) inertia_from_params(params + 10 * i, m->I[i]);
+  rnea_with_model(m, B, q, qd, qdd, tau);
+  free(m);
+  return 0;
+}
+
+/* the ten parameters of every link of the description: (m, m c, Ic + m [c]x [c]x^T) */
+int bard_oracle_inertial_params(const bard_oracle_desc* d, double* params /* [nb*10] */) {
+  omodel* m = (omodel*)malloc(sizeof(omodel));
+  int rc = build_model(d, m);
+  if (rc) { free(m); return rc; }
+  for (int i = 0; i < m->nb; ++i) {
+    const double* I = m->I[i];
+    double* th = params + 10 * i;
+    th[0] = I[3 * 6 + 3];
+    th[1] = I[2 * 6 + 4]; th[2] = I[0 * 6 + 5]; th[3] = I[1 * 6 + 3];   /* [h]x: (2,1) = hx, (0,2) = hy, (1,0) = hz */
+    th[4] = I[0]; th[5] = I[1]; th[6] = I[2]; th[7] = I[6 + 1]; th[8] = I[6 + 2]; th[9] = I[12 + 2];
+  }
+  free(m);
+  return 0;
+}
+
+int bard_oracle_rnea_vjp_params(const bard_oracle_desc* d, int64_t B, const double* q, const double* qd, const double* qdd,
+                                const double* dtau, double* dparams) {
+  omodel* m = (omodel*)malloc(sizeof(omodel));
+  int rc = build_model(d, m);
+  if (rc) { free(m); return rc; }
+  const int nb = m->nb, nv = m->nv;
+  double* tau = (double*)malloc(sizeof(double) * (size_t)(nv > 0 ? nv : 1) * (size_t)(B > 0 ? B : 1));
+  double* theta = (double*)calloc((size_t)nb * 10, sizeof(double));
+  for (int k = 0; k < nb * 10; ++k) {
+    theta[k] = 1.0;                                           /* unit parameter vector e_k */
+    for (int i = 0; i < nb; ++i) inertia_from_params(theta + 10 * i, m->I[i]);
+    rnea_with_model(m, B, q, qd, qdd, tau);                   /* = d tau / d theta_k for every environment */
+    double s = 0.0;
+    for (int64_t x = 0; x < (int64_t)nv * B; ++x) s += dtau[x] * tau[x];
+    dparams[k] = s;
+    theta[k] = 0.0;
+  }
+  free(theta);
+  free(tau);
+  free(m);
+  return 0;
+}

@@ -94,6 +94,19 @@ int  bard_oracle_body_velocity(const bard_oracle_desc* d, int64_t B, const doubl
 /* spatial inertia of body i as a dense 6x6, API order [lin; ang], row-major (free-body pin) */
 int  bard_oracle_spatial_inertia(const bard_oracle_desc* d, int32_t body, double* I66);
 
+/* RNEA as a function of the inertial parameters (the paper's system-identification use,
+ * PAPER.md:150-158).  params[nb][10] per link: m, h = m c (3), Io = Ic + m [c]x [c]x^T (xx,xy,xz,yy,yz,zz, about the
+ * BODY ORIGIN); tau is linear in them.  rnea_params = bard_oracle_rnea with the spatial inertias built from params;
+ * inertial_params = the ten parameters of the description's links; rnea_vjp_params = the VJP by its definition:
+ * dparams[k] = sum over environments and DOFs of dtau * tau(params = e_k)  (nb*10 RNEA evaluations).
+ * Pins (tests/test_rnea_vjp.py): agreement with bard_oracle_rnea at the description's parameters, linearity,
+ * pendulum closed form, central finite differences through bard_oracle_rnea with perturbed mass / COM / inertia. */
+int  bard_oracle_rnea_params(const bard_oracle_desc* d, int64_t B, const double* q, const double* qd, const double* qdd,
+                             const double* params, double* tau);
+int  bard_oracle_inertial_params(const bard_oracle_desc* d, double* params);
+int  bard_oracle_rnea_vjp_params(const bard_oracle_desc* d, int64_t B, const double* q, const double* qd, const double* qdd,
+                                 const double* dtau, double* dparams /* [nb*10] */);
+
 void bard_oracle_set_threads(int n);   /* OpenMP threads over environments; n<=0 -> all cores */
 int  bard_oracle_get_threads(void);
 

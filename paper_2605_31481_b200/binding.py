@@ -25,7 +25,7 @@ TABLES = {"LEVEL_PTR": (0, np.int32), "LEVEL_BODY": (1, np.int32), "BODY_LEVEL":
           "PARENT_SLOT": (3, np.int32), "Q_OFF": (4, np.int32), "V_OFF": (5, np.int32), "DOF_BODY": (6, np.int32),
           "ANC_MASK": (7, np.uint64), "RODRIGUES": (8, np.float32)}
 EXPORTS = ["bard_model_create", "bard_model_destroy", "bard_model_dims", "bard_model_get_table",
-           "bard_model_set_frames", "bard_model_specialize", "bard_model_specialized_source", "bard_fk", "bard_jacobian", "bard_rnea", "bard_crba", "bard_step", "bard_euler_step", "bard_aba", "bard_aba_workspace_floats",
+           "bard_model_set_frames", "bard_model_set_option", "bard_model_get_option", "bard_model_specialize", "bard_model_specialized_source", "bard_fk", "bard_jacobian", "bard_rnea", "bard_crba", "bard_step", "bard_euler_step", "bard_aba", "bard_aba_workspace_floats",
            "bard_status_string", "bard_last_error", "bard_launch_count"]
 
 
@@ -60,6 +60,8 @@ def lib():
         L.bard_model_dims.argtypes = [vp] + [C.POINTER(C.c_int32)] * 4
         L.bard_model_get_table.argtypes = [vp, C.c_int, vp, C.c_size_t, C.POINTER(C.c_size_t)]
         L.bard_model_set_frames.argtypes = [vp, C.c_int32, C.POINTER(C.c_int32), C.POINTER(C.c_double)]
+        L.bard_model_set_option.argtypes = [vp, C.c_char_p, C.c_int64]
+        L.bard_model_get_option.argtypes = [vp, C.c_char_p, C.POINTER(C.c_int64)]
         L.bard_model_specialize.argtypes = [vp, C.c_uint32]
         L.bard_model_specialized_source.argtypes = [vp, C.c_uint32, C.c_char_p, C.c_size_t, C.POINTER(C.c_size_t)]
         L.bard_fk.argtypes = [vp, i64, fp, fp, vp]
@@ -158,6 +160,15 @@ class Model:
         _check(lib().bard_model_set_frames(self._h, len(body), body.ctypes.data_as(C.POINTER(C.c_int32)),
                                            _dp(off) if off is not None else None))
         self.nframes = len(body)
+
+    def set_option(self, key: str, value: int):
+        """``bard_model_set_option``: a launch / code-generation knob of THIS model (see ``include/bard.h``)."""
+        _check(lib().bard_model_set_option(self._h, key.encode(), int(value)))
+
+    def get_option(self, key: str) -> int:
+        v = C.c_int64()
+        _check(lib().bard_model_get_option(self._h, key.encode(), C.byref(v)))
+        return int(v.value)
 
     def specialize(self, ops=("rnea",)):
         """JIT-compile model-specialised kernels for the named operators (``bard_model_specialize``)."""

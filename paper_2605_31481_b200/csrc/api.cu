@@ -2,6 +2,7 @@
 #include <cuda_runtime.h>
 
 #include <atomic>
+#include <cctype>
 #include <cstdlib>
 #include <cstring>
 #include <mutex>
@@ -27,6 +28,33 @@ namespace bard {
 static thread_local std::string g_err;
 std::atomic<int64_t> g_launches{0};
 void set_error(const std::string& s) { g_err = s; }
+
+DeviceGuard::DeviceGuard(int device) {
+  if (device < 0 || cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); return; }
+  if (prev != device) switched = cudaSetDevice(device) == cudaSuccess;
+}
+DeviceGuard::~DeviceGuard() {
+  if (switched) cudaSetDevice(prev);
+}
+
+// option name -> field; the environment default of option "x" is BARD_X
+bool option_ref(Options& o, const char* key, int64_t** ref) {
+  if (!key) return false;
+#define BARD_OPT_REF(name, dflt) if (std::strcmp(key, #name) == 0) { *ref = &o.name; return true; }
+  BARD_OPTIONS(BARD_OPT_REF)
+#undef BARD_OPT_REF
+  return false;
+}
+void options_from_env(Options& o) {
+  auto env = [](const char* name, int64_t& dst) {
+    std::string e = "BARD_";
+    for (const char* c = name; *c; ++c) e += (char)std::toupper((unsigned char)*c);
+    if (const char* v = std::getenv(e.c_str())) dst = std::atoll(v);
+  };
+#define BARD_OPT_ENV(name, dflt) env(#name, o.name);
+  BARD_OPTIONS(BARD_OPT_ENV)
+#undef BARD_OPT_ENV
+}
 bard_status build_model(const bard_model_desc* d, int device, Model& M);
 bard_status set_frames(Model& M, int32_t nframes, const int32_t* body, const double* offset);
 }  // namespace bard
@@ -115,6 +143,14 @@ bard_status bard_model_get_table(const bard_model* bm, int table_id, void* host_
 
 bard_status bard_model_set_frames(bard_model* bm, int32_t nframes, const int32_t* body, const double* offset) {
   if (!bm) { set_error("bard_model_set_frames: model is NULL"); return BARD_ERR_INVALID_ARG; }
+  if (bm->m.d_blob) {
+    // The J tables are rewritten in place and the generated Jacobian / step kernels are unloaded: nothing that reads
+    // them may still be in flight -- on the caller's streams, on non-blocking streams, or on bard_step's own side
+    // streams.  set_frames is a rare, build-time call: wait for the whole device.
+    bard::DeviceGuard guard(bm->m.device);
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) { set_error(std::string("bard_model_set_frames: ") + cudaGetErrorString(e)); cudaGetLastError(); return BARD_ERR_CUDA; }
+  }
   bard::drop_specialized_jacobian(bm->m);
   return bard::set_frames(bm->m, nframes, body, offset);
 }
@@ -122,6 +158,22 @@ bard_status bard_model_set_frames(bard_model* bm, int32_t nframes, const int32_t
 bard_status bard_model_specialize(bard_model* bm, uint32_t ops) {
   if (!bm) { set_error("bard_model_specialize: model is NULL"); return BARD_ERR_INVALID_ARG; }
   return bard::specialize(bm->m, ops);
+}
+
+bard_status bard_model_set_option(bard_model* bm, const char* key, int64_t value) {
+  if (!bm) { set_error("bard_model_set_option: model is NULL"); return BARD_ERR_INVALID_ARG; }
+  int64_t* ref = nullptr;
+  if (!bard::option_ref(bm->m.opt, key, &ref)) { set_error(std::string("bard_model_set_option: unknown option: ") + (key ? key : "(null)")); return BARD_ERR_INVALID_ARG; }
+  *ref = value;
+  return BARD_OK;
+}
+
+bard_status bard_model_get_option(const bard_model* bm, const char* key, int64_t* value) {
+  if (!bm || !value) { set_error("bard_model_get_option: NULL argument"); return BARD_ERR_INVALID_ARG; }
+  int64_t* ref = nullptr;
+  if (!bard::option_ref(const_cast<bard_model*>(bm)->m.opt, key, &ref)) { set_error(std::string("bard_model_get_option: unknown option: ") + (key ? key : "(null)")); return BARD_ERR_INVALID_ARG; }
+  *value = *ref;
+  return BARD_OK;
 }
 
 bard_status bard_model_specialized_source(const bard_model* bm, uint32_t op, char* host_dst, size_t cap, size_t* need) {
@@ -148,14 +200,17 @@ static bard_status check_call(const char* fn, const bard_model* bm, int64_t B, c
 bard_status bard_fk(const bard_model* bm, int64_t B, const float* q, float* pose, bard_stream stream) {
   bard_status s = check_call("bard_fk", bm, B, bm && bm->m.nq == 0 ? (const void*)pose : q, pose, pose, pose);
   if (s != BARD_OK || B == 0) return s;
+  bard::DeviceGuard guard(bm->m.device);
   if (bard::launch_specialized(bm->m, BARD_OP_FK, B, q, nullptr, nullptr, pose, nullptr, nullptr, nullptr, stream, s)) return s;
   return bard::launch_fk(bm->m, B, q, pose, stream);
 }
 
 bard_status bard_jacobian(const bard_model* bm, int64_t B, const float* q, float* J, bard_stream stream) {
-  if (bm && (bm->m.nframes == 0 || bm->m.nv == 0)) return check_call("bard_jacobian", bm, B, bm, bm, bm, bm);  // empty output
+  if (!bm) { set_error("bard_jacobian: model is NULL"); return BARD_ERR_INVALID_ARG; }
+  if (bm->m.nframes == 0 || bm->m.nv == 0) return check_call("bard_jacobian", bm, B, bm, bm, bm, bm);  // empty output
   bard_status s = check_call("bard_jacobian", bm, B, bm->m.nq == 0 ? (const void*)J : q, J, J, J);
   if (s != BARD_OK || B == 0) return s;
+  bard::DeviceGuard guard(bm->m.device);
   if (bard::launch_specialized(bm->m, BARD_OP_JACOBIAN, B, q, nullptr, nullptr, nullptr, J, nullptr, nullptr, stream, s)) return s;
   return bard::launch_jacobian(bm->m, B, q, J, stream);
 }
@@ -165,6 +220,7 @@ bard_status bard_rnea(const bard_model* bm, int64_t B, const float* q, const flo
   if (bm && bm->m.nv == 0) return check_call("bard_rnea", bm, B, bm, bm, bm, bm);  // nothing to write
   bard_status s = check_call("bard_rnea", bm, B, q, qd, qdd, tau);
   if (s != BARD_OK || B == 0) return s;
+  bard::DeviceGuard guard(bm->m.device);
   if (bard::launch_specialized(bm->m, BARD_OP_RNEA, B, q, qd, qdd, nullptr, nullptr, tau, nullptr, stream, s)) return s;
   return bard::launch_rnea(bm->m, B, q, qd, qdd, tau, stream);
 }
@@ -173,6 +229,7 @@ bard_status bard_crba(const bard_model* bm, int64_t B, const float* q, float* M,
   if (bm && bm->m.nv == 0) return check_call("bard_crba", bm, B, bm, bm, bm, bm);
   bard_status s = check_call("bard_crba", bm, B, q, M, M, M);
   if (s != BARD_OK || B == 0) return s;
+  bard::DeviceGuard guard(bm->m.device);
   if (bard::launch_specialized(bm->m, BARD_OP_CRBA, B, q, nullptr, nullptr, nullptr, nullptr, nullptr, M, stream, s)) return s;
   return bard::launch_crba(bm->m, B, q, M, stream);
 }
@@ -180,6 +237,7 @@ bard_status bard_crba(const bard_model* bm, int64_t B, const float* q, float* M,
 bard_status bard_step(const bard_model* bm, int64_t B, const float* q, const float* qd, const float* qdd, float* pose, float* J,
                       float* tau, float* M, bard_stream stream) {
   if (!bm) { set_error("bard_step: model is NULL"); return BARD_ERR_INVALID_ARG; }
+  bard::DeviceGuard guard(bm->m.device);
   // the fused kernel needs all four outputs to exist; otherwise (no DOF, no frames, not specialised, small batch)
   // the step is the four operators in sequence on the same stream
   if (bm->m.nv > 0 && bm->m.nframes > 0) {
@@ -191,7 +249,7 @@ bard_status bard_step(const bard_model* bm, int64_t B, const float* q, const flo
   // Small batches: one operator's grid does not fill the machine (B = 4096: 128 tiles on 148 SMs), and the four
   // operators are independent given (q, qd, qdd) -- fork them over three side streams and join, so the step costs
   // its longest operator instead of the sum.  Works under stream capture (the side streams join the capture).
-  static const int64_t fork_max_b = [] { const char* v = std::getenv("BARD_STEP_FORK_MAX_B"); return v ? std::atoll(v) : 16384ll; }();
+  const int64_t fork_max_b = bm->m.opt.step_fork_max_b;
   StepFork& f = const_cast<bard_model*>(bm)->fj;
   if (f.ok && B > 0 && B <= fork_max_b && bm->m.nv > 0) {
     std::lock_guard<std::mutex> lock(f.mu);
@@ -218,9 +276,11 @@ bard_status bard_step(const bard_model* bm, int64_t B, const float* q, const flo
 }
 
 bard_status bard_euler_step(const bard_model* bm, int64_t B, float dt, float* q, float* qd, const float* qdd, bard_stream stream) {
-  if (bm && bm->m.nq == 0) return check_call("bard_euler_step", bm, B, bm, bm, bm, bm);   // nothing to integrate
+  if (!bm) { set_error("bard_euler_step: model is NULL"); return BARD_ERR_INVALID_ARG; }
+  if (bm->m.nq == 0) return check_call("bard_euler_step", bm, B, bm, bm, bm, bm);   // nothing to integrate
   bard_status s = check_call("bard_euler_step", bm, B, q, bm->m.nv ? (const void*)qd : q, bm->m.nv ? (const void*)qdd : q, q);
   if (s != BARD_OK || B == 0) return s;
+  bard::DeviceGuard guard(bm->m.device);
   return bard::launch_euler(bm->m, B, dt, q, qd, qdd, stream);
 }
 
@@ -234,6 +294,7 @@ bard_status bard_aba(const bard_model* bm, int64_t B, const float* q, const floa
   bard_status s = check_call("bard_aba", bm, B, q, qd, tau, qdd);
   if (s == BARD_OK && B > 0 && !workspace) { set_error("bard_aba: workspace is NULL"); s = BARD_ERR_INVALID_ARG; }
   if (s != BARD_OK || B == 0) return s;
+  bard::DeviceGuard guard(bm->m.device);
   return bard::launch_aba(bm->m, B, q, qd, tau, qdd, workspace, stream);
 }
 

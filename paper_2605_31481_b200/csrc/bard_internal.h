@@ -98,8 +98,46 @@ struct JHeader {              // 8 words; byte offsets from the start of the J s
 
 struct Specialized;           // specialize.cu: model-specialised (NVRTC) kernels
 
+// Launch and code-generation knobs.  Every one is a field of the MODEL: bard_model_create reads its default from the
+// environment variable BARD_<KEY IN UPPER CASE> once, bard_model_set_option overrides it afterwards; no operator
+// call reads the environment.  -1 = "auto" (the measured rule documented next to the knob's use).
+#define BARD_OPTIONS(X)                                                                                        \
+  /* team kernels (kernels.cu) */                                                                              \
+  X(teams, 0)            /* tiles per CTA (0 = auto) */                                                        \
+  X(pack, 0)             /* force N environments per lane (1 / 2; 0 = auto) */                                 \
+  X(pack2_min_b, 32768)  /* smallest batch that runs two environments per lane */                              \
+  X(pdl, 1)              /* programmatic dependent launch attribute on every launch */                         \
+  /* which kernel family a call gets (specialize.cu, api.cu) */                                                \
+  X(spec_min_b, -1)            /* smallest batch for the plain specialised kernels */                          \
+  X(spec_block, 0)             /* force the CTA size of the specialised kernels */                             \
+  X(spec_roles_max_b, -1)      /* largest batch for the limb-role RNEA */                                      \
+  X(spec_crba_roles_max_b, -1) /* largest / smallest batch for the limb-role CRBA */                           \
+  X(spec_crba_roles_min_b, -1)                                                                                 \
+  X(spec_fused_max_rows, 112)  /* the fused step kernel is used at every batch up to this many parked rows */  \
+  X(spec_fused_small_b, -1)    /* ... and above it only up to this batch */                                    \
+  X(spec_kin_min_b, -1)        /* smallest batch at which bard_step uses the kinematics-fused kernel + RNEA */ \
+  X(step_fork_max_b, 16384)    /* bard_step forks the four operators over side streams up to this batch */     \
+  /* read by bard_model_specialize (code generation) */                                                        \
+  X(spec_prefetch, 2)          /* bodies of input-load lookahead */                                            \
+  X(spec_sync, -1)             /* bodies between CTA barriers (0 = none) */                                    \
+  X(spec_l2pf, -1)             /* up-front L2 prefetch: 0 never, 1 always, 2 two kernels */                    \
+  X(spec_roles, 2)             /* limb roles */                                                                \
+  X(spec_zero_role, 1)         /* CRBA limb roles: a group of warps that only stores M's structural zeros */   \
+  X(spec_maxreg, 0)            /* --maxrregcount of the NVRTC compile (0 = none) */                            \
+  X(spec_step4, 1)             /* build the side-by-side step kernel */                                        \
+  X(spec_step4_max_rows, 72)                                                                                   \
+  X(spec_pair, -1)             /* RNEA: pack two components of one environment's 3-vectors per FFMA2 */
+struct Options {
+#define BARD_OPT_FIELD(name, dflt) int64_t name = dflt;
+  BARD_OPTIONS(BARD_OPT_FIELD)
+#undef BARD_OPT_FIELD
+};
+void options_from_env(Options& o);
+bool option_ref(Options& o, const char* key, int64_t** ref);
+
 struct Model {
   int device = 0;
+  Options opt;
   Specialized* spec = nullptr;
   int32_t nb = 0, nq = 0, nv = 0, nlevels = 0, nslots = 0, nframes = 0, nfree = 0;
   int32_t team_warps = 1;             // L: warps that share one 32-environment tile (level-parallel schedule)
@@ -116,6 +154,23 @@ struct Model {
   void* d_jblob = nullptr;            // J (allocated for the largest frame set)
   size_t common_bytes = 0, m_bytes = 0, j_bytes = 0;
   int sm_count = 148;
+  // where rnea_kernel parks the staged input rows (shared-memory row of q / qd / qdd row r); built once with the model
+  uint16_t rowmap_q[128] = {}, rowmap_qd[64] = {}, rowmap_qdd[64] = {};
+  // fp64 copy of the per-body constants (the fp32 BodyConst rows are these, rounded once): R0 A B t0 a b (36),
+  // Sw Sl (6), mass, h (3), Io (6) = 52 doubles per body; gravity.  Read by the fp64 code generator.
+  std::vector<double> bc64;
+  double g64[3] = {0, 0, 0};
+  std::vector<double> frame_off64;    // nframes * 3
+};
+constexpr int kBc64 = 52;
+
+// Makes the model's device current for the duration of a call (and restores the caller's): one cudaGetDevice, and a
+// cudaSetDevice only when a process drives several GPUs and the caller's current device is another one.
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(int device);
+  ~DeviceGuard();
 };
 
 constexpr size_t kJBlobMax = sizeof(JHeader) + sizeof(FrameConst) * BARD_MAX_FRAMES +

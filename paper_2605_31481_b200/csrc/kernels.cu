@@ -29,6 +29,7 @@
 #include <atomic>
 #include <cstdint>
 #include <cstdlib>
+#include <cstring>
 #include <type_traits>
 
 #include "bard_internal.h"
@@ -933,24 +934,21 @@ __global__ void __launch_bounds__(256) euler_kernel(const unsigned char* __restr
 }
 
 // ----------------------------------------------------------------------------- launchers
-struct LaunchCfg { int teams, threads, team_rows, pack; size_t smem; unsigned grid; uint32_t rcpL; };
+struct LaunchCfg { int teams, threads, team_rows, pack; size_t smem; unsigned grid; uint32_t rcpL; bool pdl = true; };
 
 constexpr size_t kSmemMax = 227 * 1024;
 
-int env_int(const char* name, int dflt) {
-  const char* v = std::getenv(name);
-  return v ? std::atoi(v) : dflt;
-}
 bool aligned(const void* p, uintptr_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) == 0; }
 
 // N (environments per lane): 2 when the batch is even, every pointer is 8-byte aligned, there are enough
 // tiles to fill the machine and the doubled tile state still leaves three CTAs per SM; else 1.  TEAMS per CTA: two tiles share one copy of the constants when the team
 // is narrow; fewer if the state does not fit.  Small CTAs keep the last wave short.
-bool pick_cfg(int L, int64_t B, size_t const_bytes, int team_rows, bool can_pack2, int64_t max_rows,
+bool pick_cfg(const Options& o, int L, int64_t B, size_t const_bytes, int team_rows, bool can_pack2, int64_t max_rows,
               LaunchCfg& cfg, std::string& why) {
-  const int want_teams = env_int("BARD_TEAMS", 0);             // tuning / test knobs (read per call)
-  const int want_pack = env_int("BARD_PACK", 0);
-  const int pack2_min_b = env_int("BARD_PACK2_MIN_B", 32768);
+  const int want_teams = (int)o.teams;                         // tuning / test knobs: fields of the model (bard_model_set_option)
+  const int want_pack = (int)o.pack;
+  const int64_t pack2_min_b = o.pack2_min_b;
+  cfg.pdl = o.pdl != 0;
   const size_t fixed = 16 + const_bytes;
   // two environments per lane halve the non-FP instructions per environment but double the tile's shared
   // memory: taken only when at least three such CTAs still fit on an SM (measured: DESIGN.md "Tuning")
@@ -1005,7 +1003,6 @@ template <int V> using IC = std::integral_constant<int, V>;
 // Launch with programmatic stream serialization (PDL): see setup().
 template <typename K, typename... Args>
 void launch(K kernel, const LaunchCfg& cfg, void* stream, Args... args) {
-  static const int pdl = env_int("BARD_PDL", 1);
   cudaLaunchConfig_t lc = {};
   lc.gridDim = dim3(cfg.grid);
   lc.blockDim = dim3(cfg.threads);
@@ -1015,7 +1012,7 @@ void launch(K kernel, const LaunchCfg& cfg, void* stream, Args... args) {
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   lc.attrs = attr;
-  lc.numAttrs = pdl ? 1 : 0;
+  lc.numAttrs = cfg.pdl ? 1 : 0;
   cudaLaunchKernelEx(&lc, kernel, args...);
 }
 
@@ -1029,6 +1026,7 @@ void launch(K kernel, const LaunchCfg& cfg, void* stream, Args... args) {
 bard_status launch_euler(const Model& m, int64_t B, float dt, float* q, float* qd, const float* qdd, void* stream) {
   if ((int64_t)std::max(m.nq, m.nv) * B >= ((int64_t)1 << 32)) return refuse("bard_euler_step", "an input array has 2^32 elements or more");
   LaunchCfg cfg = {};
+  cfg.pdl = m.opt.pdl != 0;
   cfg.threads = 256;
   cfg.grid = (unsigned)((B + 255) / 256);
   cfg.smem = 0;
@@ -1039,7 +1037,7 @@ bard_status launch_fk(const Model& m, int64_t B, const float* q, float* pose, vo
   LaunchCfg cfg;
   std::string why;
   const bool p2 = B % 2 == 0 && aligned(q, 8) && aligned(pose, 8);
-  if (!pick_cfg(m.team_warps, B, m.common_bytes, m.nq + 12 * m.nslots, p2, std::max(12 * m.nb, m.nq), cfg, why)) return refuse("bard_fk", why);
+  if (!pick_cfg(m.opt, m.team_warps, B, m.common_bytes, m.nq + 12 * m.nslots, p2, std::max(12 * m.nb, m.nq), cfg, why)) return refuse("bard_fk", why);
   auto go = [&](auto kernel, auto id) {
     bard_status s = prep<decltype(id)::value>(kernel, "bard_fk");
     if (s != BARD_OK) return s;
@@ -1053,7 +1051,7 @@ bard_status launch_jacobian(const Model& m, int64_t B, const float* q, float* J,
   LaunchCfg cfg;
   std::string why;
   const bool p2 = B % 2 == 0 && aligned(q, 8) && aligned(J, 8);
-  if (!pick_cfg(m.team_warps, B, m.common_bytes + m.j_bytes, m.nq + 12 * m.nslots + 6 * m.nv + 3 * m.nframes, p2,
+  if (!pick_cfg(m.opt, m.team_warps, B, m.common_bytes + m.j_bytes, m.nq + 12 * m.nslots + 6 * m.nv + 3 * m.nframes, p2,
                 std::max(6 * m.nframes * m.nv, m.nq), cfg, why))
     return refuse("bard_jacobian", why);
   const int vec_ok = (B % 4 == 0) && aligned(J, 16);
@@ -1071,19 +1069,13 @@ bard_status launch_rnea(const Model& m, int64_t B, const float* q, const float* 
   LaunchCfg cfg;
   std::string why;
   const bool p2 = B % 2 == 0 && aligned(q, 8) && aligned(qd, 8) && aligned(qdd, 8) && aligned(tau, 8);
-  if (!pick_cfg(m.team_warps, B, m.common_bytes, 12 * m.nslots + 8 * m.nb + 19 * m.nfree, p2, std::max(m.nq, m.nv), cfg, why))
+  if (!pick_cfg(m.opt, m.team_warps, B, m.common_bytes, 12 * m.nslots + 8 * m.nb + 19 * m.nfree, p2, std::max(m.nq, m.nv), cfg, why))
     return refuse("bard_rnea", why);
-  RowMap map;                                                  // where the staged input rows land (see rnea_kernel)
-  for (int i = 0; i < m.nb; ++i) {
-    const int reg = 12 * m.nslots + 8 * i, qo = m.q_off[i], vo = m.v_off[i];
-    if (m.jtype[i] == BARD_JOINT_FREE) {
-      const int fi = 12 * m.nslots + 8 * m.nb + 19 * m.free_index[i];
-      for (int k = 0; k < 7; ++k) map.q[qo + k] = (uint16_t)(fi + k);
-      for (int k = 0; k < 6; ++k) { map.qd[vo + k] = (uint16_t)(fi + 7 + k); map.qdd[vo + k] = (uint16_t)(fi + 13 + k); }
-    } else if (m.jtype[i] != BARD_JOINT_FIXED) {
-      map.q[qo] = (uint16_t)(reg + 6); map.qd[vo] = (uint16_t)reg; map.qdd[vo] = (uint16_t)(reg + 1);
-    }
-  }
+  RowMap map;                                                  // where the staged input rows land: built once with the model
+  static_assert(sizeof(map.q) == sizeof(m.rowmap_q) && sizeof(map.qd) == sizeof(m.rowmap_qd) && sizeof(map.qdd) == sizeof(m.rowmap_qdd), "RowMap");
+  std::memcpy(map.q, m.rowmap_q, sizeof(map.q));
+  std::memcpy(map.qd, m.rowmap_qd, sizeof(map.qd));
+  std::memcpy(map.qdd, m.rowmap_qdd, sizeof(map.qdd));
   auto go = [&](auto kernel, auto id) {
     bard_status s = prep<decltype(id)::value>(kernel, "bard_rnea");
     if (s != BARD_OK) return s;
@@ -1097,7 +1089,7 @@ bard_status launch_crba(const Model& m, int64_t B, const float* q, float* M, voi
   LaunchCfg cfg;
   std::string why;
   const bool p2 = B % 2 == 0 && aligned(q, 8) && aligned(M, 8);
-  if (!pick_cfg(m.crba_warps, B, m.common_bytes + m.m_bytes, m.nq + 12 * m.nslots + 6 * m.nv + 10 * m.nb + 12 * m.nfree, p2,
+  if (!pick_cfg(m.opt, m.crba_warps, B, m.common_bytes + m.m_bytes, m.nq + 12 * m.nslots + 6 * m.nv + 10 * m.nb + 12 * m.nfree, p2,
                 std::max(m.nv * m.nv, m.nq), cfg, why))
     return refuse("bard_crba", why);
   const int vec_ok = (B % 4 == 0) && aligned(M, 16);

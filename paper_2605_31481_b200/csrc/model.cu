@@ -83,7 +83,9 @@ bard_status build_model(const bard_model_desc* d, int device, Model& M) {
       set_error("bard_model_create: parent[i] must be in {-1, 0..i-1}");
       return BARD_ERR_TOPOLOGY;
     }
-    if (!(d->mass[i] > 0.0)) { set_error("bard_model_create: mass must be positive"); return BARD_ERR_INVALID_ARG; }
+    // mass >= 0: massless links (URDF base / tool / sensor frames behind fixed joints) are legal for FK, Jacobian,
+    // RNEA and CRBA; only ABA needs a positive-definite articulated inertia under every DOF (checked there)
+    if (!(d->mass[i] >= 0.0)) { set_error("bard_model_create: mass must be >= 0"); return BARD_ERR_INVALID_ARG; }
     if ((t == BARD_JOINT_REVOLUTE || t == BARD_JOINT_PRISMATIC)) {
       if (!d->axis) { set_error("bard_model_create: axis is NULL"); return BARD_ERR_INVALID_ARG; }
       const double* a = d->axis + 3 * i;
@@ -98,6 +100,7 @@ bard_status build_model(const bard_model_desc* d, int device, Model& M) {
     }
   }
   M.device = device;
+  options_from_env(M.opt);
   M.nb = nb;
   M.parent.assign(d->parent, d->parent + nb);
   M.jtype.assign(d->joint_type, d->joint_type + nb);
@@ -330,6 +333,8 @@ bard_status build_model(const bard_model_desc* d, int device, Model& M) {
   }
   BodyConst* BC = reinterpret_cast<BodyConst*>(M.blob.data() + sizeof(BlobHeader));
   M.rodrigues.assign((size_t)nb * 36, 0.f);
+  M.bc64.assign((size_t)nb * kBc64, 0.0);
+  for (int k = 0; k < 3; ++k) M.g64[k] = d->gravity[k];
   M.free_index.assign(nb, -1);
   for (int i = 0; i < nb; ++i) {
     BodyConst& c = BC[i];
@@ -379,6 +384,10 @@ bard_status build_model(const bard_model_desc* d, int device, Model& M) {
     put(&M.rodrigues[(size_t)36 * i], rod, 36);
     put(c.Sw, Sw, 3);
     put(c.Sl, Sl, 3);
+    double* c64 = &M.bc64[(size_t)kBc64 * i];
+    std::memcpy(c64, rod, sizeof(rod));
+    std::memcpy(c64 + 36, Sw, sizeof(Sw));
+    std::memcpy(c64 + 39, Sl, sizeof(Sl));
     // compact spatial inertia about the body origin: m, h = m c, Io = Ic + m (|c|^2 1 - c c^T)
     const double m = d->mass[i];
     const double* cm = d->com + 3 * i;
@@ -390,6 +399,9 @@ bard_status build_model(const bard_model_desc* d, int device, Model& M) {
     c.mass = (float)m;
     put(c.h, h, 3);
     put(c.Io, Io, 6);
+    c64[42] = m;
+    std::memcpy(c64 + 43, h, sizeof(h));
+    std::memcpy(c64 + 46, Io, sizeof(Io));
     c.type = t; c.parent = M.parent[i]; c.q_off = M.q_off[i]; c.v_off = M.v_off[i];
     c.src = src[i]; c.save = save[i]; c.flags = post_id ? 1 : 0; c.level = M.body_level[i];
     if (t == BARD_JOINT_FREE) { M.free_index[i] = M.nfree; c.flags |= (M.nfree++) << 8; }
@@ -397,6 +409,17 @@ bard_status build_model(const bard_model_desc* d, int device, Model& M) {
     c.child_begin = child_begin[i]; c.child_count = (int32_t)children[i].size();
   }
 
+  // where rnea_kernel parks the staged input rows: in the rows that later hold the body's force (see rnea_kernel)
+  for (int i = 0; i < nb; ++i) {
+    const int reg = 12 * nslots + 8 * i, qo = M.q_off[i], vo = M.v_off[i];
+    if (M.jtype[i] == BARD_JOINT_FREE) {
+      const int fi = 12 * nslots + 8 * nb + 19 * M.free_index[i];
+      for (int k = 0; k < 7 && qo + k < 128; ++k) M.rowmap_q[qo + k] = (uint16_t)(fi + k);
+      for (int k = 0; k < 6; ++k) { M.rowmap_qd[vo + k] = (uint16_t)(fi + 7 + k); M.rowmap_qdd[vo + k] = (uint16_t)(fi + 13 + k); }
+    } else if (M.jtype[i] != BARD_JOINT_FIXED) {
+      M.rowmap_q[qo] = (uint16_t)(reg + 6); M.rowmap_qd[vo] = (uint16_t)reg; M.rowmap_qdd[vo] = (uint16_t)(reg + 1);
+    }
+  }
   set_frames(M, 0, nullptr, nullptr);   // empty J section (host side; the device copy follows below)
   if (device < 0) return BARD_OK;  // host-only model: tables can be queried, operators refuse to run
   int dev_count = 0;
@@ -472,6 +495,8 @@ bard_status set_frames(Model& M, int32_t nframes, const int32_t* body, const dou
   if (!zrows.empty()) std::memcpy(M.jblob.data() + off_zrows, zrows.data(), sizeof(uint16_t) * zrows.size());
   M.j_bytes = bytes;
   M.nframes = nframes;
+  M.frame_off64.assign((size_t)nframes * 3, 0.0);
+  for (int k = 0; k < 3 * nframes && offset; ++k) M.frame_off64[k] = offset[k];
   if (!M.d_jblob) return BARD_OK;
   int prev = 0;
   cudaGetDevice(&prev);

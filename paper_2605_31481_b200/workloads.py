@@ -1,9 +1,11 @@
 """Seeded synthetic robots and states (the ONLY module shared by the CUDA path's tests/bench and the oracle's).
 
-It holds none of the method's arithmetic: no kinematics, no dynamics, no level schedule.  It only draws the
-inputs both sides consume -- robot descriptions (topology, joint types/axes, fixed offsets, inertial
+It holds none of the method's arithmetic: no kinematics, no dynamics, no integrator, no level schedule.  It only
+draws the inputs both sides consume -- robot descriptions (topology, joint types/axes, fixed offsets, inertial
 parameters) and batches of (q, qd, qdd) -- with ``numpy.random.default_rng`` (PCG64), following the recipe
-of BASELINE.json ``configs`` as restated in SURVEY.md section 8(d) and DESIGN.md "Input recipe".
+of BASELINE.json ``configs`` as restated in SURVEY.md section 8(d) and DESIGN.md "Input recipe".  (The one formula
+here, ``_quat_to_R``, turns a drawn unit quaternion into the rotation part of a FIXED offset of the description;
+the numpy manifold step the tests use as a finite-difference stencil lives in ``tests/manifold.py``.)
 
 These robots stand in for the paper's URDF models (xArm7 / SPARC / Go2 / G1), which are not
 available; only their shapes (DOF count, tree topology, depth) are taken.
@@ -240,48 +242,3 @@ def sample_states(desc: RobotDesc, B: int, seed: int, dtype=np.float32, zero_qd=
 def config_states(cfg: int, B: int, step: int = 0, dtype=np.float32):
     """State seed 2000 + config (+ step), SURVEY 8(d)."""
     return sample_states(config_robot(cfg), B, seed=2000 + cfg + 100 * step, dtype=dtype)
-
-
-def manifold_step(desc: RobotDesc, q: np.ndarray, dv: np.ndarray) -> np.ndarray:
-    """q (+) dv: revolute/prismatic add; free base p += R(quat) v, quat += 1/2 quat (x) (omega, 0), renormalised.
-    ``dv`` is a tangent increment (already multiplied by dt), layout [nv, B].  Used to roll config 2 forward
-    (explicit Euler) and for finite-difference test stencils."""
-    q = np.array(q, dtype=np.float64, copy=True)
-    qo, vo = desc.q_off, desc.v_off
-    for i, t in enumerate(desc.joint_type):
-        t = int(t)
-        if t in (REVOLUTE, PRISMATIC):
-            q[qo[i]] += dv[vo[i]]
-        elif t == FREE:
-            x, y, z, w = q[qo[i] + 3:qo[i] + 7]
-            n = np.sqrt(x * x + y * y + z * z + w * w)
-            x, y, z, w = x / n, y / n, z / n, w / n
-            v, om = dv[vo[i]:vo[i] + 3], dv[vo[i] + 3:vo[i] + 6]
-            R = _quat_to_R(x, y, z, w)  # [3,3,B]
-            q[qo[i]:qo[i] + 3] += np.einsum("ijb,jb->ib", R, v)
-            # quaternion product quat (x) (om, 0): body-frame angular increment
-            ox, oy, oz = om
-            dx = 0.5 * (w * ox + y * oz - z * oy)
-            dy = 0.5 * (w * oy + z * ox - x * oz)
-            dz = 0.5 * (w * oz + x * oy - y * ox)
-            dw = 0.5 * (-x * ox - y * oy - z * oz)
-            nq4 = np.stack([x + dx, y + dy, z + dz, w + dw])
-            nq4 /= np.linalg.norm(nq4, axis=0, keepdims=True)
-            q[qo[i] + 3:qo[i] + 7] = nq4
-    return q
-
-
-def euler_rollout(cfg: int, B: int, steps: int = 24, dt: float = 0.005, dtype=np.float32):
-    """config 2 style trajectory: per step fresh seeded qdd, qd += dt qdd, q (+)= dt qd.  Returns a list of
-    (q, qd, qdd) per step, each rounded once to ``dtype`` (the state carried forward stays fp64)."""
-    desc = config_robot(cfg)
-    q, qd, _ = sample_states(desc, B, seed=2000 + cfg, dtype=np.float64)
-    out = []
-    for s in range(steps):
-        rng = np.random.default_rng(2000 + cfg + 100 * (s + 1))
-        qdd = rng.normal(size=(desc.nv, B))
-        out.append((np.ascontiguousarray(q.astype(dtype)), np.ascontiguousarray(qd.astype(dtype)),
-                    np.ascontiguousarray(qdd.astype(dtype))))
-        qd = qd + dt * qdd
-        q = manifold_step(desc, q, dt * qd)
-    return out

@@ -5,6 +5,7 @@ import pytest
 from scipy.spatial.transform import Rotation
 
 import oracle
+import manifold
 from paper_2605_31481_b200 import binding, workloads as W
 
 
@@ -15,14 +16,14 @@ def nerr(x, ref):
 # ------------------------------------------------------------------------------------------- oracle pins (CPU)
 @pytest.mark.parametrize("cfg", [0, 1, 2, 3])
 def test_oracle_step_agrees_with_the_independent_numpy_formulation(cfg):
-    """oracle (C, rotation from the FK routine's quaternion matrix) vs workloads.manifold_step (numpy, written
+    """oracle (C, rotation from the FK routine's quaternion matrix) vs tests/manifold.py manifold_step (numpy, written
     separately for the finite-difference stencils): two formulations of the same step."""
     desc = W.config_robot(cfg)
     o = oracle.Oracle(desc)
     q, qd, qdd = W.sample_states(desc, 64, seed=11 + cfg, dtype=np.float64)
     q1, qd1 = o.euler_step(0.005, q, qd, qdd)
     qd2 = qd + 0.005 * qdd
-    q2 = W.manifold_step(desc, q, 0.005 * qd2)
+    q2 = manifold.manifold_step(desc, q, 0.005 * qd2)
     assert np.abs(qd1 - qd2).max() == 0.0
     assert np.abs(q1 - q2).max() <= 1e-15
 
@@ -92,15 +93,15 @@ def test_gpu_euler_step_matches_oracle(idx, B):
 
 
 @pytest.mark.gpu
-def test_config2_rollout_on_the_device(monkeypatch):
+def test_config2_rollout_on_the_device():
     """config 2 as BASELINE.json states it: 24 consecutive steps, all four operators per step (bard_step), q
     advanced on the DEVICE by bard_euler_step from seeded qdd; the oracle integrates the same qdd in fp64.  The
     operators are compared at every step on the device trajectory (rounded to the oracle's input), and the two
     trajectories must stay together (fp32 drift only)."""
-    monkeypatch.setenv("BARD_SPEC_MIN_B", "0")
     cfg, B, dt = 2, 512, 0.005
     desc = W.config_robot(cfg)
     m = binding.Model(desc, device=0)
+    m.set_option("spec_min_b", 0)
     m.specialize(("fk", "jacobian", "rnea", "crba", "fused"))
     o = oracle.Oracle(desc)
     dev = torch.device("cuda:0")

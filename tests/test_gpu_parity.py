@@ -5,6 +5,7 @@ import numpy as np
 import pytest
 
 import oracle
+import manifold
 from paper_2605_31481_b200 import binding, workloads as W
 
 torch = pytest.importorskip("torch")
@@ -85,6 +86,34 @@ def test_random_trees_all_joint_types(seed):
     Gpu(desc).check(q, qd, qdd)
 
 
+def massless_fixed_links(seed, nb=9, free_root=False):
+    """A tree whose FIXED-joint bodies are massless frames (URDF base / tool / sensor links), incl. a massless leaf."""
+    desc = W.random_tree(seed, nb=nb, joint_types=(W.REVOLUTE, W.FIXED, W.PRISMATIC), free_root=free_root, nframes=3)
+    jt = desc.joint_type.copy()
+    jt[nb - 1] = W.FIXED                                # a massless tool frame at a leaf
+    if not free_root:
+        jt[0] = W.FIXED                                 # a massless base link
+    desc.joint_type = jt
+    for i in range(nb):
+        if int(jt[i]) == W.FIXED:
+            desc.mass[i] = 0.0
+            desc.com[i] = 0.0
+            desc.inertia[i] = 0.0
+    return desc
+
+
+@pytest.mark.parametrize("seed", range(4))
+def test_massless_fixed_links(seed):
+    """bodies with mass 0 (frames behind fixed joints) are legal for FK, Jacobian, RNEA and CRBA."""
+    desc = massless_fixed_links(820 + seed, free_root=(seed % 2 == 1))
+    q, qd, qdd = W.sample_states(desc, 300, seed=3 + seed)
+    g = Gpu(desc)
+    g.check(q, qd, qdd)
+    g.m.set_option("spec_min_b", 0)
+    g.m.specialize(("fk", "jacobian", "rnea", "crba"))
+    g.check(q, qd, qdd)
+
+
 def test_max_size_tree():
     desc = W.random_tree(4242, nb=64, shape="random", nframes=16)
     q, qd, qdd = W.sample_states(desc, 96, seed=5)
@@ -121,7 +150,7 @@ def test_euler_rollout_config2():
     """config 2: 24 consecutive steps, q advanced by explicit Euler from random qdd; all four operators per step."""
     desc = W.config_robot(2)
     g = Gpu(desc)
-    for q, qd, qdd in W.euler_rollout(2, 256, steps=24):
+    for q, qd, qdd in manifold.euler_rollout(2, 256, steps=24):
         g.check(q, qd, qdd)
 
 
@@ -154,19 +183,26 @@ def test_full_size_sampled(cfg, B):
         assert np.isfinite(a).all()
 
 
-@pytest.mark.parametrize("knobs", [{"BARD_PACK": "2"}, {"BARD_PACK": "1"}, {"BARD_PACK": "2", "BARD_FORCE_GENERAL": "1"},
-                                   {"BARD_TEAM_WARPS": "1"}, {"BARD_TEAM_WARPS": "8", "BARD_PACK": "2"},
-                                   {"BARD_TEAMS": "1"}])
+@pytest.mark.parametrize("knobs", [{"pack": 2}, {"pack": 1}, {"pack": 2, "BARD_FORCE_GENERAL": "1"},
+                                   {"BARD_TEAM_WARPS": "1"}, {"BARD_TEAM_WARPS": "8", "pack": 2},
+                                   {"teams": 1}])
 @pytest.mark.parametrize("cfg", [0, 1, 2, 3])
 def test_every_kernel_instantiation(cfg, knobs, monkeypatch):
     """The launch heuristics pick (environments per lane, SIMPLE/general kernels, team width) from B and the
-    model; the test knobs force each instantiation on every config, at a size with several tiles and a ragged tail."""
+    model; the test knobs force each instantiation on every config, at a size with several tiles and a ragged tail.
+    Launch knobs are model options; the two that shape the model's constant tables (team width, general kernels)
+    are read from the environment once, by bard_model_create."""
     for k, v in knobs.items():
-        monkeypatch.setenv(k, v)
+        if k.startswith("BARD_"):
+            monkeypatch.setenv(k, v)
     desc = W.config_robot(cfg)
     for B in (1000, 130):
         q, qd, qdd = W.config_states(cfg, B)
-        Gpu(desc).check(q, qd, qdd)
+        g = Gpu(desc)
+        for k, v in knobs.items():
+            if not k.startswith("BARD_"):
+                g.m.set_option(k, v)
+        g.check(q, qd, qdd)
 
 
 def test_odd_batch_and_misaligned_views():

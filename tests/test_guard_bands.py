@@ -31,17 +31,18 @@ class Banded:
 
 @pytest.mark.parametrize("cfg,B", [(3, 1000 + 13), (1, 97), (0, 4096 + 1), (2, 33)])
 @pytest.mark.parametrize("path", ["team", "specialised", "fused", "side_by_side"])
-def test_no_write_outside_the_outputs(cfg, B, path, monkeypatch):
-    monkeypatch.setenv("BARD_SPEC_MIN_B", str(1 << 30) if path == "team" else "0")
-    if path == "fused":
-        monkeypatch.setenv("BARD_SPEC_FUSED_MAX_ROWS", "100000")
-    if path == "side_by_side":
-        monkeypatch.setenv("BARD_SPEC_FUSED_MAX_ROWS", "0")
-        monkeypatch.setenv("BARD_SPEC_FUSED_SMALL_B", "0")
-        monkeypatch.setenv("BARD_SPEC_STEP4_MAX_ROWS", "100000")
+def test_no_write_outside_the_outputs(cfg, B, path):
     desc = W.config_robot(cfg)
     dev = torch.device("cuda:0")
     m = binding.Model(desc, device=0)
+    m.set_option("spec_min_b", (1 << 30) if path == "team" else 0)
+    if path == "fused":
+        m.set_option("spec_fused_max_rows", 100000)
+    if path == "side_by_side":
+        m.set_option("spec_fused_max_rows", 0)
+        m.set_option("spec_fused_small_b", 0)
+        m.set_option("spec_step4_max_rows", 100000)
+        m.set_option("spec_kin_min_b", 1 << 40)
     if path != "team":
         m.specialize(("fk", "jacobian", "rnea", "crba") + (("fused",) if path != "specialised" else ()))
     q, qd, qdd = W.config_states(cfg, B)

@@ -76,9 +76,14 @@ def test_validation_errors():
     assert ei.value.code == 1
     bad = W.config_robot(0)
     bad.mass = bad.mass.copy()
-    bad.mass[2] = 0.0
+    bad.mass[2] = -1.0
     with pytest.raises(binding.BardError):
         binding.Model(bad, device=-1)
+    bad.mass[2] = float("nan")
+    with pytest.raises(binding.BardError):
+        binding.Model(bad, device=-1)
+    bad.mass[2] = 0.0                                # a massless link is legal (URDF frames behind fixed joints)
+    binding.Model(bad, device=-1).close()
     bad = W.config_robot(0)
     bad.axis = bad.axis.copy()
     bad.axis[1] = 0.0
@@ -103,3 +108,34 @@ def test_free_joint_requires_identity_T_post():
     d.T_post[0, 3] = 0.1
     with pytest.raises(binding.BardError):
         binding.Model(d, device=-1)
+
+
+def test_options_are_fields_of_the_model_and_null_handles_are_refused(monkeypatch):
+    """Knobs live in the model: the environment gives the default ONCE at bard_model_create, set_option overrides it,
+    another model is unaffected; unknown keys and NULL handles return BARD_ERR_INVALID_ARG (never a crash)."""
+    monkeypatch.setenv("BARD_SPEC_MIN_B", "777")
+    a = binding.Model(W.config_robot(0), device=-1)
+    monkeypatch.delenv("BARD_SPEC_MIN_B")
+    b = binding.Model(W.config_robot(0), device=-1)
+    assert a.get_option("spec_min_b") == 777 and b.get_option("spec_min_b") == -1
+    a.set_option("spec_min_b", 5)
+    assert a.get_option("spec_min_b") == 5 and b.get_option("spec_min_b") == -1
+    with pytest.raises(binding.BardError) as ei:
+        a.set_option("no_such_knob", 1)
+    assert ei.value.code == 1
+    L = binding.lib()
+    import ctypes as C
+    v = C.c_int64()
+    null = C.c_void_p()
+    assert L.bard_model_set_option(null, b"pack", 1) == 1
+    assert L.bard_model_get_option(null, b"pack", C.byref(v)) == 1
+    # every operator entry point with a NULL model: an error code, not a segfault
+    assert L.bard_fk(null, 4, None, None, None) == 1
+    assert L.bard_jacobian(null, 4, None, None, None) == 1
+    assert L.bard_rnea(null, 4, None, None, None, None, None) == 1
+    assert L.bard_crba(null, 4, None, None, None) == 1
+    assert L.bard_step(null, 4, None, None, None, None, None, None, None, None) == 1
+    assert L.bard_euler_step(null, 4, 0.01, None, None, None, None) == 1
+    assert L.bard_aba(null, 4, None, None, None, None, None, None) == 1
+    assert L.bard_model_set_frames(null, 0, None, None) == 1
+    assert L.bard_model_specialize(null, 1) == 1

@@ -10,6 +10,7 @@ import pytest
 from scipy.spatial.transform import Rotation
 
 import oracle
+import manifold
 from paper_2605_31481_b200 import workloads as W
 
 G = 9.81
@@ -154,7 +155,7 @@ def fd_jacobian(o, d, q, h=1e-6):
     for k in range(o.nv):
         dv = np.zeros((o.nv, B))
         dv[k] = h
-        Pp, Pm = o.fk(W.manifold_step(d, q, dv)), o.fk(W.manifold_step(d, q, -dv))
+        Pp, Pm = o.fk(manifold.manifold_step(d, q, dv)), o.fk(manifold.manifold_step(d, q, -dv))
         for f, body in enumerate(d.frame_body):
             Rp, Rm = Pp[body, :9].reshape(3, 3, B), Pm[body, :9].reshape(3, 3, B)
             pe_p = Pp[body, 9:] + np.einsum("ijb,j->ib", Rp, offs[f])
@@ -301,7 +302,7 @@ def test_rnea_gravity_only_equals_potential_gradient():
     for k in range(o.nv):
         dv = np.zeros((o.nv, B))
         dv[k] = h
-        np.testing.assert_allclose(tau[k], (U(W.manifold_step(d, q, dv)) - U(W.manifold_step(d, q, -dv))) / (2 * h), atol=2e-8)
+        np.testing.assert_allclose(tau[k], (U(manifold.manifold_step(d, q, dv)) - U(manifold.manifold_step(d, q, -dv))) / (2 * h), atol=2e-8)
 
 
 # ----------------------------------------------------------------------------- tables: brute force
@@ -355,5 +356,5 @@ def test_coriolis_power_equals_kinetic_energy_rate(mk):
     power = np.einsum("ib,ib->b", qd, o.rnea(q, qd, z) - o.rnea(q, z, z))
     h = 1e-6
     T = lambda qq: 0.5 * np.einsum("ib,ijb,jb->b", qd, o.crba(qq), qd)
-    dT = (T(W.manifold_step(d, q, h * qd)) - T(W.manifold_step(d, q, -h * qd))) / (2 * h)
+    dT = (T(manifold.manifold_step(d, q, h * qd)) - T(manifold.manifold_step(d, q, -h * qd))) / (2 * h)
     np.testing.assert_allclose(power, dT, atol=1e-7 * max(1.0, np.abs(dT).max()))

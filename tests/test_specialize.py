@@ -86,12 +86,12 @@ def _single_root_and_branches(desc):
     return parent.count(-1) == 1 and any(n >= 2 for n in nchild)
 
 
-def test_limb_role_source_on_a_host_only_model(monkeypatch):
+def test_limb_role_source_on_a_host_only_model():
     """The limb-role RNEA kernel is generated where a single-rooted tree branches, one `if (role == r)` stretch per
     role, forces handed over through park_to and one named barrier; never for a chain."""
     for roles in (2, 3):
-        monkeypatch.setenv("BARD_SPEC_ROLES", str(roles))
         m = binding.Model(W.config_robot(3), device=-1)
+        m.set_option("spec_roles", roles)
         m.specialize(("rnea",))
         src = m.specialized_source("rnea_roles")
         for r in range(roles):
@@ -104,7 +104,7 @@ def test_limb_role_source_on_a_host_only_model(monkeypatch):
         m.specialized_source("rnea_roles")
 
 
-def test_rnea_source_has_a_variant_without_l2_prefetch(monkeypatch):
+def test_rnea_source_has_a_variant_without_l2_prefetch():
     """RNEA is generated twice by default: with the up-front L2 prefetch (grids of one wave) and without it
     (`_np`, larger grids); BARD_SPEC_L2PF = 1 / 0 generate one kernel; the other operators always one."""
     m = binding.Model(W.config_robot(1), device=-1)
@@ -113,8 +113,8 @@ def test_rnea_source_has_a_variant_without_l2_prefetch(monkeypatch):
     assert "bard_rnea_n1_np(" in src and "bard_rnea_n1(" in src and "if (PF) {" in src
     assert "_np(" not in m.specialized_source("fk")
     for v in ("0", "1"):
-        monkeypatch.setenv("BARD_SPEC_L2PF", v)
         m = binding.Model(W.config_robot(1), device=-1)
+        m.set_option("spec_l2pf", int(v))
         m.specialize(("rnea",))
         src = m.specialized_source("rnea")
         assert "_np(" not in src and ("pf_l2(q" in src) == (v == "1")
@@ -125,12 +125,28 @@ torch = pytest.importorskip("torch")
 
 
 class Spec:
-    def __init__(self, desc, ops=ALL):
+    def __init__(self, desc, ops=ALL, **opts):
+        """`opts`: knobs of THIS model, set through bard_model_set_option before the kernels are generated."""
         assert torch.cuda.is_available(), "GPU tests need CUDA; there is no CPU fallback"
         self.m = binding.Model(desc, device=0)
+        for k, v in opts.items():
+            self.m.set_option(k, v)
         self.m.specialize(ops)
         self.o = oracle.Oracle(desc)
         self.dev = torch.device("cuda:0")
+
+    def run_dev(self, q, qd, qdd):
+        """As run(), but the outputs stay on the device (full bench sizes: gigabytes)."""
+        m, B, dev = self.m, q.shape[1], self.dev
+        tq, tqd, tqdd = (torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in (q, qd, qdd))
+        outs = [torch.full(sh, float("nan"), device=dev) for sh in ((m.nb, 12, B), (m.nframes, 6, m.nv, B), (m.nv, B), (m.nv, m.nv, B))]
+        s = torch.cuda.current_stream().cuda_stream
+        m.fk(B, tq, outs[0], s)
+        m.jacobian(B, tq, outs[1], s)
+        m.rnea(B, tq, tqd, tqdd, outs[2], s)
+        m.crba(B, tq, outs[3], s)
+        torch.cuda.synchronize()
+        return outs
 
     def run(self, q, qd, qdd):
         """All four operators, NaN-filled outputs (every element must be overwritten), one launch each."""
@@ -166,20 +182,19 @@ class Spec:
 @pytest.mark.gpu
 @pytest.mark.parametrize("idx", range(10))
 @pytest.mark.parametrize("B", [1, 37, 1000])
-def test_specialized_operators_match_oracle(idx, B, monkeypatch):
-    monkeypatch.setenv("BARD_SPEC_MIN_B", "0")                    # the specialised kernels at every batch size
+def test_specialized_operators_match_oracle(idx, B):
     desc = _robots()[idx]
-    s = Spec(desc)
+    s = Spec(desc, spec_min_b=0)                                  # the specialised kernels at every batch size
     q, qd, qdd = W.sample_states(desc, B, seed=900 + idx)
     out = s.run(q, qd, qdd)
     ref = s.refs(q, qd, qdd)
     s.check(out, ref)                                             # RNEA here: limb roles where the tree branches
-    monkeypatch.setenv("BARD_SPEC_ROLES_MAX_B", "0")              # RNEA and CRBA: one thread per environment
-    monkeypatch.setenv("BARD_SPEC_CRBA_ROLES_MAX_B", "0")
+    s.m.set_option("spec_roles_max_b", 0)                         # RNEA and CRBA: one thread per environment
+    s.m.set_option("spec_crba_roles_max_b", 0)
     out = s.run(q, qd, qdd)
     s.check(out, ref)
     # and the team kernels on the same inputs: same arithmetic up to the folded zeros
-    monkeypatch.setenv("BARD_SPEC_MIN_B", str(1 << 30))
+    s.m.set_option("spec_min_b", 1 << 30)
     team = s.run(q, qd, qdd)
     for a, b in zip(out, team):
         assert nerr(a, b.astype(np.float64)) <= 1e-4
@@ -188,17 +203,14 @@ def test_specialized_operators_match_oracle(idx, B, monkeypatch):
 @pytest.mark.gpu
 @pytest.mark.parametrize("block", [0, 32, 96, 512])
 @pytest.mark.parametrize("roles_max_b", [None, 0])
-def test_specialized_block_sizes_and_ragged_tail(block, roles_max_b, monkeypatch):
+def test_specialized_block_sizes_and_ragged_tail(block, roles_max_b):
     """Any block size (a run-time value) and a batch that ends in the middle of a warp; RNEA with limb roles
     (the default at this batch size) and without."""
-    monkeypatch.setenv("BARD_SPEC_MIN_B", "0")
-    if block:
-        monkeypatch.setenv("BARD_SPEC_BLOCK", str(block))
+    opts = {"spec_min_b": 0, "spec_block": block}
     if roles_max_b is not None:
-        monkeypatch.setenv("BARD_SPEC_ROLES_MAX_B", str(roles_max_b))
-        monkeypatch.setenv("BARD_SPEC_CRBA_ROLES_MAX_B", str(roles_max_b))
+        opts.update(spec_roles_max_b=roles_max_b, spec_crba_roles_max_b=roles_max_b)
     desc = W.config_robot(3)
-    s = Spec(desc)
+    s = Spec(desc, **opts)
     q, qd, qdd = W.config_states(3, 5000 + 13)
     s.check(s.run(q, qd, qdd), s.refs(q, qd, qdd))
 
@@ -206,13 +218,11 @@ def test_specialized_block_sizes_and_ragged_tail(block, roles_max_b, monkeypatch
 @pytest.mark.gpu
 @pytest.mark.parametrize("roles", [2, 3, 4])
 @pytest.mark.parametrize("idx", range(10))
-def test_limb_role_rnea_matches_oracle(roles, idx, monkeypatch):
+def test_limb_role_rnea_matches_oracle(roles, idx):
     """RNEA with the subtrees below the first branching body dealt to `roles` groups of warps: against the oracle,
     below the specialised regime too (its own rule), and it never runs above its batch limit."""
-    monkeypatch.setenv("BARD_SPEC_ROLES", str(roles))             # read when the kernel is generated
-    monkeypatch.setenv("BARD_SPEC_MIN_B", str(1 << 30))           # roles have their own regime
     desc = _robots()[idx]
-    s = Spec(desc, ops=("rnea",))
+    s = Spec(desc, ops=("rnea",), spec_roles=roles, spec_min_b=1 << 30)   # roles have their own regime
     dev = torch.device("cuda:0")
     try:
         branching = "role == 1u" in s.m.specialized_source("rnea_roles")
@@ -225,10 +235,7 @@ def test_limb_role_rnea_matches_oracle(roles, idx, monkeypatch):
         ref = s.o.rnea(*(np.ascontiguousarray(a.astype(np.float64)) for a in (q, qd, qdd)))
         got = {}
         for mx in (None, 0):
-            if mx is None:
-                monkeypatch.delenv("BARD_SPEC_ROLES_MAX_B", raising=False)
-            else:
-                monkeypatch.setenv("BARD_SPEC_ROLES_MAX_B", str(mx))
+            s.m.set_option("spec_roles_max_b", -1 if mx is None else mx)   # -1: the library's own rule
             tau = torch.full((s.m.nv, B), float("nan"), device=dev)
             s.m.rnea(B, tq, tqd, tqdd, tau, torch.cuda.current_stream().cuda_stream)
             torch.cuda.synchronize()
@@ -242,14 +249,12 @@ def test_limb_role_rnea_matches_oracle(roles, idx, monkeypatch):
 @pytest.mark.gpu
 @pytest.mark.parametrize("roles", [2, 3])
 @pytest.mark.parametrize("idx", range(10))
-def test_limb_role_crba_matches_oracle(roles, idx, monkeypatch):
+def test_limb_role_crba_matches_oracle(roles, idx):
     """CRBA with limb roles (composite inertias of the other roles' subtrees handed over in the world frame, rows of a
     subtree's DOFs against the trunk filled by the subtree's role): every entry of M written, symmetric bit for bit,
     against the oracle and against the one-thread-per-environment kernel."""
-    monkeypatch.setenv("BARD_SPEC_ROLES", str(roles))             # read when the kernel is generated
-    monkeypatch.setenv("BARD_SPEC_MIN_B", "0")
     desc = _robots()[idx]
-    s = Spec(desc, ops=("crba",))
+    s = Spec(desc, ops=("crba",), spec_roles=roles, spec_min_b=0)
     dev = torch.device("cuda:0")
     try:
         branching = "role == 1u" in s.m.specialized_source("crba_roles")
@@ -262,8 +267,8 @@ def test_limb_role_crba_matches_oracle(roles, idx, monkeypatch):
         ref = s.o.crba(np.ascontiguousarray(q.astype(np.float64)))
         got = {}
         for mx in (1 << 30, 0):
-            monkeypatch.setenv("BARD_SPEC_CRBA_ROLES_MAX_B", str(mx))
-            monkeypatch.setenv("BARD_SPEC_CRBA_ROLES_MIN_B", "0")
+            s.m.set_option("spec_crba_roles_max_b", mx)
+            s.m.set_option("spec_crba_roles_min_b", 0)
             Mo = torch.full((s.m.nv, s.m.nv, B), float("nan"), device=dev)
             s.m.crba(B, tq, Mo, torch.cuda.current_stream().cuda_stream)
             torch.cuda.synchronize()
@@ -278,13 +283,11 @@ def test_limb_role_crba_matches_oracle(roles, idx, monkeypatch):
 
 @pytest.mark.gpu
 @pytest.mark.parametrize("idx", [0, 1, 2, 4, 5, 7, 9])
-def test_fused_step_matches_oracle_and_the_four_calls(idx, monkeypatch):
+def test_fused_step_matches_oracle_and_the_four_calls(idx):
     """bard_step: one fused kernel where it is built (small parked state), else the four operators; both against
     the oracle, and the fused outputs against the four specialised kernels bit for bit (same generated arithmetic)."""
-    monkeypatch.setenv("BARD_SPEC_MIN_B", "0")
-    monkeypatch.setenv("BARD_SPEC_FUSED_MAX_ROWS", "100000")      # build the fused kernel for every robot here
     desc = _robots()[idx]
-    s = Spec(desc)
+    s = Spec(desc, spec_min_b=0, spec_fused_max_rows=100000)      # build the fused kernel for every robot here
     s.m.specialize(("fused",))
     q, qd, qdd = W.sample_states(desc, 700, seed=40 + idx)
     four = s.run(q, qd, qdd)
@@ -303,15 +306,12 @@ def test_fused_step_matches_oracle_and_the_four_calls(idx, monkeypatch):
 
 @pytest.mark.gpu
 @pytest.mark.parametrize("cfg,B", [(3, 1000), (2, 777), (3, 65536)])
-def test_side_by_side_step_is_one_launch_and_bit_equal_to_the_four_kernels(cfg, B, monkeypatch):
+def test_side_by_side_step_is_one_launch_and_bit_equal_to_the_four_kernels(cfg, B):
     """Where the fused kernel does not pay, bard_step is ONE launch of the four specialised operators side by side
     (blockIdx.y = operator): the same generated code, so the same bits as the four separate launches."""
-    monkeypatch.setenv("BARD_SPEC_MIN_B", "0")
-    monkeypatch.setenv("BARD_SPEC_FUSED_MAX_ROWS", "0")           # never the fused kernel ...
-    monkeypatch.setenv("BARD_SPEC_FUSED_SMALL_B", "0")            # ... at any batch size
-    monkeypatch.setenv("BARD_SPEC_STEP4_MAX_ROWS", "100000")      # build the side-by-side kernel for every robot here
     desc = W.config_robot(cfg)
-    s = Spec(desc)
+    # never the fused kernel, at any batch size; build the side-by-side kernel for every robot here
+    s = Spec(desc, spec_min_b=0, spec_fused_max_rows=0, spec_fused_small_b=0, spec_step4_max_rows=100000, spec_kin_min_b=1 << 40)
     s.m.specialize(("fused",))
     q, qd, qdd = W.config_states(cfg, B)
     four = s.run(q, qd, qdd)
@@ -346,15 +346,15 @@ def test_step_without_specialisation_is_the_four_team_kernels():
 
 
 @pytest.mark.gpu
-def test_specialized_max_size_tree_and_single_fixed_body(monkeypatch):
+def test_specialized_max_size_tree_and_single_fixed_body():
     """The compiled limits (64 bodies, 16 frames) and the degenerate model (one fixed body: no q, no DOF)."""
-    monkeypatch.setenv("BARD_SPEC_MIN_B", "0")
     desc = W.random_tree(4242, nb=64, shape="random", nframes=16)
-    s = Spec(desc)
+    s = Spec(desc, spec_min_b=0)
     q, qd, qdd = W.sample_states(desc, 96, seed=5)
     s.check(s.run(q, qd, qdd), s.refs(q, qd, qdd))
     one = W.build_robot("one_fixed", [-1], [W.FIXED], seed=1)
     m = binding.Model(one, device=0)
+    m.set_option("spec_min_b", 0)
     m.specialize(ALL + ("fused",))
     pose = torch.full((1, 12, 8), float("nan"), device="cuda:0")
     n0 = binding.launch_count()
@@ -365,10 +365,9 @@ def test_specialized_max_size_tree_and_single_fixed_body(monkeypatch):
 
 
 @pytest.mark.gpu
-def test_specialized_jacobian_follows_set_frames(monkeypatch):
-    monkeypatch.setenv("BARD_SPEC_MIN_B", "0")
+def test_specialized_jacobian_follows_set_frames():
     desc = W.config_robot(3)
-    s = Spec(desc)
+    s = Spec(desc, spec_min_b=0)
     q, qd, qdd = W.config_states(3, 257)
     s.check(s.run(q, qd, qdd), s.refs(q, qd, qdd))
     desc.frame_body = [5, 23, 14]                                  # new frames: team kernel until specialised again
@@ -382,41 +381,128 @@ def test_specialized_jacobian_follows_set_frames(monkeypatch):
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("cfg,B", [(3, 65536), (1, 65536), (2, 65536), (0, 1048576)])
+@pytest.mark.parametrize("cfg,B", [(3, 65536), (1, 65536), (2, 65536), (0, 1048576), (3, 262144), (3, 1048576), (1, 1048576),
+                                   (2, 1048576), (0, 65536), (0, 262144)])
 def test_specialized_full_size_sampled(cfg, B):
-    """bench.py's launch configuration (default knobs): a strided sample of environments against the oracle."""
+    """bench.py's launch configuration (default knobs, every size of BASELINE.json's sweep from 65 536 up, where the
+    launch rule changes: one wave of 448-thread CTAs -> multi-wave 256-thread CTAs and the RNEA variant without L2
+    prefetch): a strided sample of environments against the oracle, every output element finite, repeat bit-identical.
+    The outputs stay on the device (7.7 GB for the humanoid at 1 Mi); only the sampled columns come to the host."""
     desc = W.config_robot(cfg)
     s = Spec(desc)
     q, qd, qdd = W.config_states(cfg, B)
-    out = s.run(q, qd, qdd)
-    idx = np.unique(np.concatenate([np.arange(0, B, max(1, B // 997)), [B - 1, B - 2, 127, 128, B // 2]]))
+    out = s.run_dev(q, qd, qdd)
+    # the sample: a stride that is coprime to the warp / CTA sizes, the ragged ends, CTA boundaries of both launch shapes
+    idx = np.unique(np.concatenate([np.arange(0, B, max(1, B // 997)), [B - 1, B - 2, 127, 128, 255, 256, 447, 448, B // 2]]))
     ref = s.refs(*(a[:, idx] for a in (q, qd, qdd)))
+    tidx = torch.from_numpy(idx).to(s.dev)
     for a in out:
-        assert np.isfinite(a).all()
+        assert bool(torch.isfinite(a).all())
     for a, r, tol in zip(out, ref, (TOL_KIN, TOL_KIN, TOL_DYN, TOL_DYN)):
-        assert nerr(a[..., idx], r) <= tol
-    again = s.run(q, qd, qdd)
-    for a, b in zip(out, again):
-        assert np.array_equal(a, b)                                # no atomics, fixed child order
+        assert nerr(a.index_select(a.dim() - 1, tidx).cpu().numpy(), r) <= tol
+    assert bool(torch.equal(out[3], out[3].transpose(0, 1)))       # M symmetric bit for bit, all B environments
+    cs = [a.view(torch.int32).sum(dtype=torch.int64).item() for a in out]   # bit pattern checksums: a repeat must match
+    again = s.run_dev(q, qd, qdd)
+    for a, b, c in zip(out, again, cs):
+        assert b.view(torch.int32).sum(dtype=torch.int64).item() == c   # no atomics, fixed child order
+        if a.numel() < (1 << 28):
+            assert bool(torch.equal(a, b))
+
+
+def wide_states(desc, B, seed):
+    """Revolute angles far outside (-pi, pi) (continuous joints wind up): U(-200 pi, 200 pi), and in the first
+    environments exact multiples of pi/2, +-1e4 rad, +-1e5 rad -- the range reduction of the kernels' own sincos
+    runs with every quadrant and large k (reading 16)."""
+    q, qd, qdd = W.sample_states(desc, B, seed=seed)
+    rng = np.random.default_rng(seed + 1)
+    special = np.array([0.0, np.pi / 2, -np.pi / 2, np.pi, -np.pi, 1.5 * np.pi, 2 * np.pi, 100 * np.pi, -99.5 * np.pi, 1e4, -1e4, 1e5, -1e5,
+                        12345.678, -54321.0, 200 * np.pi], np.float64)
+    qo = desc.q_off
+    for i, t in enumerate(desc.joint_type):
+        if int(t) == W.REVOLUTE:
+            row = rng.uniform(-200 * np.pi, 200 * np.pi, size=B)
+            k = min(B, len(special))
+            row[:k] = np.roll(special, i)[:k]
+            q[qo[i]] = row.astype(np.float32)
+    return q, qd, qdd
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("idx", range(10))
+def test_wide_angles_both_kernel_families(idx):
+    """every other parity input is U(-pi, pi); here the hand-written sincos (3-step Cody-Waite
+    reduction) sees |q| up to 1e5 in the team kernels, the specialised kernels and the limb-role kernels."""
+    desc = _robots()[idx]
+    s = Spec(desc, spec_min_b=0)
+    for B in (1000, 37):
+        q, qd, qdd = wide_states(desc, B, seed=5100 + idx)
+        ref = s.refs(q, qd, qdd)
+        s.m.set_option("spec_min_b", 0)
+        s.m.set_option("spec_roles_max_b", -1)
+        s.m.set_option("spec_crba_roles_max_b", -1)
+        s.check(s.run(q, qd, qdd), ref)                            # specialised, limb roles where the tree branches
+        s.m.set_option("spec_roles_max_b", 0)
+        s.m.set_option("spec_crba_roles_max_b", 0)
+        s.check(s.run(q, qd, qdd), ref)                            # specialised, one thread per environment
+        s.m.set_option("spec_min_b", 1 << 30)
+        s.check(s.run(q, qd, qdd), ref)                            # team kernels
+        s.m.set_option("pack", 2)
+        s.check(s.run(q, qd, qdd), ref)                            # team kernels, two environments per lane (packed sincos)
+        s.m.set_option("pack", 0)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("family", ["team", "team_pack2", "specialised"])
+def test_sincos_of_the_kernels_against_fp64(family):
+    """The kernels' own sincos, isolated: FK of ONE revolute joint about z with T_pre = I gives R = Rz(q), so
+    pose[3] = R10 = 0 + sin q * 1 is the kernel's sine bit for bit and pose[0] = R00 = 1 - (1 - cos q) its cosine after
+    two roundings of at most half an ulp of 1 each (6e-8 + 6e-8).  Claim (reading 16): |error| <= 9.4e-8 for
+    |q| <= 1e6 rad.  Checked over 2 Mi angles: uniform in +-1e5, log-uniform magnitudes down to 1e-6, and a comb around
+    every multiple of pi/2 up to 2000 pi (where a wrong reduction constant shows first)."""
+    B = 1 << 21
+    rng = np.random.default_rng(99)
+    n = B // 4
+    comb = (np.arange(n) % 4001 - 2000)[:, None] * (np.pi / 2) + rng.uniform(-1e-3, 1e-3, size=(n, 1))
+    q = np.concatenate([rng.uniform(-1e5, 1e5, size=n), rng.uniform(-np.pi, np.pi, size=n),
+                        np.sign(rng.normal(size=n)) * 10.0 ** rng.uniform(-6, 6, size=n), comb[:, 0]]).astype(np.float32)[None, :]
+    T = np.zeros((1, 12)); T[0, 0] = T[0, 5] = T[0, 10] = 1.0
+    desc = W.RobotDesc(name="rz", parent=np.array([-1], np.int32), joint_type=np.array([W.REVOLUTE], np.int32),
+                       axis=np.array([[0.0, 0.0, 1.0]]), T_pre=T, T_post=None, mass=np.array([1.0]), com=np.zeros((1, 3)),
+                       inertia=np.array([[1.0, 0, 0, 1.0, 0, 1.0]]))
+    m = binding.Model(desc, device=0)
+    if family == "specialised":
+        m.set_option("spec_min_b", 0)
+        m.specialize(("fk",))
+    elif family == "team_pack2":
+        m.set_option("pack", 2)
+    dev = torch.device("cuda:0")
+    pose = torch.full((1, 12, B), float("nan"), device=dev)
+    m.fk(B, torch.from_numpy(q).to(dev), pose, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    p = pose.cpu().numpy().astype(np.float64)[0]
+    q64 = q[0].astype(np.float64)
+    assert np.max(np.abs(p[3] - np.sin(q64))) <= 9.4e-8            # R10 = sin q
+    assert np.max(np.abs(p[1] + np.sin(q64))) <= 9.4e-8            # R01 = -sin q
+    assert np.max(np.abs(p[0] - np.cos(q64))) <= 9.4e-8 + 1.2e-7   # R00 = 1 - (1 - cos q)
+    assert np.max(np.abs(p[4] - np.cos(q64))) <= 9.4e-8 + 1.2e-7
+    assert np.array_equal(p[8], np.ones(B)) and not p[[2, 5, 6, 7, 9, 10, 11]].any()
 
 
 @pytest.mark.gpu
 @pytest.mark.parametrize("cfg", [1, 3])
-def test_rnea_variant_without_l2_prefetch_matches(cfg, monkeypatch):
+def test_rnea_variant_without_l2_prefetch_matches(cfg):
     """Grids beyond two CTAs per SM run the RNEA variant without the L2 prefetch (here forced with 32-thread CTAs):
     same arithmetic, so bit-identical to the prefetching variant, and within tolerance of the oracle."""
-    monkeypatch.setenv("BARD_SPEC_MIN_B", "0")
-    monkeypatch.setenv("BARD_SPEC_ROLES_MAX_B", "0")
     desc = W.config_robot(cfg)
-    s = Spec(desc, ops=("rnea",))
+    s = Spec(desc, ops=("rnea",), spec_min_b=0, spec_roles_max_b=0)
     B = 32 * 2 * 148 + 32 * 40 + 7                                 # > 2 x SMs CTAs of 32 threads, ragged tail
     q, qd, qdd = W.sample_states(desc, B, seed=4242 + cfg)
     o = s.o
     ref = o.rnea(q.astype(np.float64), qd.astype(np.float64), qdd.astype(np.float64))
     tq, tqd, tqdd = (torch.from_numpy(np.ascontiguousarray(a)).to(s.dev) for a in (q, qd, qdd))
     taus = []
-    for block in ("32", "512"):                                    # 337 CTAs (no prefetch) / 22 CTAs (prefetch)
-        monkeypatch.setenv("BARD_SPEC_BLOCK", block)
+    for block in (32, 512):                                        # 337 CTAs (no prefetch) / 22 CTAs (prefetch)
+        s.m.set_option("spec_block", block)
         tau = torch.full((s.m.nv, B), float("nan"), device=s.dev)
         s.m.rnea(B, tq, tqd, tqdd, tau, torch.cuda.current_stream().cuda_stream)
         torch.cuda.synchronize()
