@@ -190,6 +190,25 @@ size_t      bard_aba_workspace_floats(const bard_model* m, int64_t B);
 bard_status bard_aba(const bard_model* m, int64_t B, const float* q, const float* qd, const float* tau, float* qdd,
                      float* workspace, bard_stream stream);
 
+/* Reverse-mode derivative of RNEA with respect to the inertial parameters (the paper's
+ * differentiable "functional mode", and its use: link masses identified through RNEA).
+ * theta[nb][10] per link: m, h = m c (3), Io = Ic + m [c]x [c]x^T (xx,xy,xz,yy,yz,zz about the BODY ORIGIN, body axes);
+ * tau is linear in theta.  Given the loss cotangent dtau[nv][B] (device, SoA like tau):
+ *   dparams[i][k] = sum_b sum_j dtau[j][b] * d tau[j][b] / d theta[i][k]            (device, [nb*10] floats, fully overwritten)
+ * One outward pass per environment (dtau is pushed outward like a velocity; no inward pass), then a DETERMINISTIC batch
+ * reduction: fixed butterfly inside a warp, warps and CTAs summed in ascending order (the last stage in fp64) -- the
+ * same bits on every call with the same B.  Table-driven, any model, no bard_model_specialize needed; two launches.
+ * `workspace`: caller-owned device buffer of bard_rnea_vjp_workspace_floats(model, B) floats.  B == 0 writes zeros. */
+size_t      bard_rnea_vjp_workspace_floats(const bard_model* m, int64_t B);
+bard_status bard_rnea_vjp_params(const bard_model* m, int64_t B, const float* q, const float* qd, const float* qdd,
+                                 const float* dtau, float* dparams, float* workspace, bard_stream stream);
+/* The model's theta (HOST, [nb*10] doubles) as bard_model_create derived it from (mass, com, inertia) -- and its
+ * replacement, for optimisation loops over the inertial parameters (system identification): a build-time call like
+ * bard_model_set_frames (SYNCHRONISES the device, rewrites the constant tables, drops the generated RNEA / CRBA / step /
+ * ABA kernels, which have theta folded in as literals: the team kernels serve until bard_model_specialize runs again). */
+bard_status bard_model_inertial_params(const bard_model* m, double* host_params);
+bard_status bard_model_set_inertial_params(bard_model* m, const double* host_params);
+
 const char* bard_status_string(bard_status s);
 const char* bard_last_error(void);
 /* Number of kernel launches this process has enqueued through the library (bench.py's gpu_launches). */

@@ -25,7 +25,8 @@ TABLES = {"LEVEL_PTR": (0, np.int32), "LEVEL_BODY": (1, np.int32), "BODY_LEVEL":
           "PARENT_SLOT": (3, np.int32), "Q_OFF": (4, np.int32), "V_OFF": (5, np.int32), "DOF_BODY": (6, np.int32),
           "ANC_MASK": (7, np.uint64), "RODRIGUES": (8, np.float32)}
 EXPORTS = ["bard_model_create", "bard_model_destroy", "bard_model_dims", "bard_model_get_table",
-           "bard_model_set_frames", "bard_model_set_option", "bard_model_get_option", "bard_model_specialize", "bard_model_specialized_source", "bard_fk", "bard_jacobian", "bard_rnea", "bard_crba", "bard_step", "bard_euler_step", "bard_aba", "bard_aba_workspace_floats",
+           "bard_model_set_frames", "bard_model_set_option", "bard_model_get_option", "bard_model_specialize", "bard_model_specialized_source", "bard_fk", "bard_jacobian", "bard_rnea", "bard_crba", "bard_step", "bard_euler_step", "bard_aba", "bard_aba_workspace_floats", "bard_rnea_vjp_params", "bard_rnea_vjp_workspace_floats",
+           "bard_model_inertial_params", "bard_model_set_inertial_params",
            "bard_status_string", "bard_last_error", "bard_launch_count"]
 
 
@@ -73,6 +74,11 @@ def lib():
         L.bard_aba.argtypes = [vp, i64, fp, fp, fp, fp, fp, vp]
         L.bard_aba_workspace_floats.argtypes = [vp, i64]
         L.bard_aba_workspace_floats.restype = C.c_size_t
+        L.bard_rnea_vjp_workspace_floats.argtypes = [vp, i64]
+        L.bard_rnea_vjp_workspace_floats.restype = C.c_size_t
+        L.bard_rnea_vjp_params.argtypes = [vp, i64, fp, fp, fp, fp, fp, fp, vp]
+        L.bard_model_inertial_params.argtypes = [vp, C.POINTER(C.c_double)]
+        L.bard_model_set_inertial_params.argtypes = [vp, C.POINTER(C.c_double)]
         L.bard_status_string.argtypes = [C.c_int]
         L.bard_status_string.restype = C.c_char_p
         L.bard_last_error.restype = C.c_char_p
@@ -217,6 +223,23 @@ class Model:
     def aba(self, B, q, qd, tau, qdd, workspace, stream=0):
         """Forward dynamics qdd = M^-1 (tau - C) (``bard_aba``); needs ``specialize(("aba",))`` first."""
         _check(lib().bard_aba(self._h, int(B), _ptr(q), _ptr(qd), _ptr(tau), _ptr(qdd), _ptr(workspace), stream or None))
+
+    def rnea_vjp_workspace_floats(self, B) -> int:
+        return int(lib().bard_rnea_vjp_workspace_floats(self._h, int(B)))
+
+    def rnea_vjp_params(self, B, q, qd, qdd, dtau, dparams, workspace, stream=0):
+        """dparams[nb, 10] = sum_b (d tau_b / d theta)^T dtau_b (``bard_rnea_vjp_params``), theta = (m, m c, Io) per link."""
+        _check(lib().bard_rnea_vjp_params(self._h, int(B), _ptr(q), _ptr(qd), _ptr(qdd), _ptr(dtau), _ptr(dparams),
+                                          _ptr(workspace), stream or None))
+
+    def inertial_params(self) -> np.ndarray:
+        out = np.zeros((self.nb, 10))
+        _check(lib().bard_model_inertial_params(self._h, _dp(out)))
+        return out
+
+    def set_inertial_params(self, params):
+        p = _f64(params, (self.nb, 10))
+        _check(lib().bard_model_set_inertial_params(self._h, _dp(p)))
 
     def crba(self, B, q, M, stream=0):
         _check(lib().bard_crba(self._h, int(B), _ptr(q), _ptr(M), stream or None))

@@ -298,6 +298,62 @@ bard_status bard_aba(const bard_model* bm, int64_t B, const float* q, const floa
   return bard::launch_aba(bm->m, B, q, qd, tau, qdd, workspace, stream);
 }
 
+size_t bard_rnea_vjp_workspace_floats(const bard_model* bm, int64_t B) {
+  return (bm && B > 0) ? bard::rnea_vjp_workspace_floats(bm->m, B) : 0;
+}
+
+bard_status bard_rnea_vjp_params(const bard_model* bm, int64_t B, const float* q, const float* qd, const float* qdd, const float* dtau,
+                                 float* dparams, float* workspace, bard_stream stream) {
+  if (!bm) { set_error("bard_rnea_vjp_params: model is NULL"); return BARD_ERR_INVALID_ARG; }
+  if (!dparams) { set_error("bard_rnea_vjp_params: dparams is NULL"); return BARD_ERR_INVALID_ARG; }
+  bard_status s = check_call("bard_rnea_vjp_params", bm, B, bm->m.nq ? (const void*)q : dparams, bm->m.nv ? (const void*)qd : dparams,
+                             bm->m.nv ? (const void*)qdd : dparams, bm->m.nv ? (const void*)dtau : dparams);
+  if (s == BARD_OK && B > 0 && !workspace) { set_error("bard_rnea_vjp_params: workspace is NULL"); s = BARD_ERR_INVALID_ARG; }
+  if (s != BARD_OK) return s;
+  bard::DeviceGuard guard(bm->m.device);
+  if (B == 0) {                                             // the sum over no environments
+    cudaError_t e = cudaMemsetAsync(dparams, 0, sizeof(float) * 10 * (size_t)bm->m.nb, (cudaStream_t)stream);
+    if (e != cudaSuccess) { set_error(std::string("bard_rnea_vjp_params: ") + cudaGetErrorString(e)); cudaGetLastError(); return BARD_ERR_CUDA; }
+    return BARD_OK;
+  }
+  return bard::launch_rnea_vjp(bm->m, B, q, qd, qdd, dtau, dparams, workspace, stream);
+}
+
+bard_status bard_model_inertial_params(const bard_model* bm, double* host_params) {
+  if (!bm || !host_params) { set_error("bard_model_inertial_params: NULL argument"); return BARD_ERR_INVALID_ARG; }
+  for (int i = 0; i < bm->m.nb; ++i)
+    for (int k = 0; k < 10; ++k) host_params[10 * i + k] = bm->m.bc64[(size_t)bard::kBc64 * i + 42 + k];
+  return BARD_OK;
+}
+
+bard_status bard_model_set_inertial_params(bard_model* bm, const double* host_params) {
+  if (!bm || !host_params) { set_error("bard_model_set_inertial_params: NULL argument"); return BARD_ERR_INVALID_ARG; }
+  bard::Model& m = bm->m;
+  for (int k = 0; k < 10 * m.nb; ++k)
+    if (!(host_params[k] == host_params[k])) { set_error("bard_model_set_inertial_params: NaN parameter"); return BARD_ERR_INVALID_ARG; }
+  bard::DeviceGuard guard(m.device);
+  if (m.d_blob) {                                            // as bard_model_set_frames: nothing that reads the tables may be in flight
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) { set_error(std::string("bard_model_set_inertial_params: ") + cudaGetErrorString(e)); cudaGetLastError(); return BARD_ERR_CUDA; }
+  }
+  bard::drop_specialized_dynamics(m);
+  bard::BodyConst* BC = reinterpret_cast<bard::BodyConst*>(m.blob.data() + sizeof(bard::BlobHeader));
+  for (int i = 0; i < m.nb; ++i) {
+    const double* th = host_params + 10 * i;
+    double* c64 = &m.bc64[(size_t)bard::kBc64 * i];
+    for (int k = 0; k < 10; ++k) c64[42 + k] = th[k];
+    BC[i].mass = (float)th[0];
+    for (int k = 0; k < 3; ++k) BC[i].h[k] = (float)th[1 + k];
+    for (int k = 0; k < 6; ++k) BC[i].Io[k] = (float)th[4 + k];
+  }
+  if (m.d_blob) {
+    const size_t bytes = sizeof(bard::BlobHeader) + sizeof(bard::BodyConst) * (size_t)m.nb;
+    cudaError_t e = cudaMemcpy(m.d_blob, m.blob.data(), bytes, cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { set_error(std::string("bard_model_set_inertial_params: ") + cudaGetErrorString(e)); cudaGetLastError(); return BARD_ERR_CUDA; }
+  }
+  return BARD_OK;
+}
+
 const char* bard_status_string(bard_status s) {
   switch (s) {
     case BARD_OK: return "BARD_OK";

@@ -195,6 +195,12 @@ const std::string* specialized_source(const Model& M, uint32_t op);
 bool launch_specialized(const Model& M, uint32_t op, int64_t B, const float* q, const float* qd, const float* qdd, float* pose,
                         float* J, float* tau, float* Mo, void* stream, bard_status& st);
 void drop_specialized_jacobian(Model& M);
+void drop_specialized_dynamics(Model& M);      // kernels with the inertial parameters folded in as literals
+
+// vjp.cu
+size_t rnea_vjp_workspace_floats(const Model& M, int64_t B);
+bard_status launch_rnea_vjp(const Model& M, int64_t B, const float* q, const float* qd, const float* qdd, const float* dtau,
+                            float* dparams, float* ws, void* stream);
 bard_status launch_aba(const Model& M, int64_t B, const float* q, const float* qd, const float* tau, float* qdd, float* ws, void* stream);
 
 }  // namespace bard

@@ -358,3 +358,18 @@ def test_coriolis_power_equals_kinetic_energy_rate(mk):
     T = lambda qq: 0.5 * np.einsum("ib,ijb,jb->b", qd, o.crba(qq), qd)
     dT = (T(manifold.manifold_step(d, q, h * qd)) - T(manifold.manifold_step(d, q, -h * qd))) / (2 * h)
     np.testing.assert_allclose(power, dT, atol=1e-7 * max(1.0, np.abs(dT).max()))
+
+
+def test_oracle_under_asan_ubsan(tmp_path):
+    """SURVEY section 5 (sanitizers row): every entry point of the oracle under AddressSanitizer + UBSan on a small tree
+    with all four joint types (tests/oracle_asan_driver.c).  A report aborts the driver with a non-zero exit code."""
+    import os
+    import subprocess
+    here = os.path.dirname(os.path.abspath(__file__))
+    exe = str(tmp_path / "oracle_asan")
+    subprocess.run(["gcc", "-std=c99", "-O1", "-g", "-fopenmp", "-fsanitize=address,undefined", "-fno-sanitize-recover=all",
+                    "-fno-omit-frame-pointer", "-o", exe, os.path.join(here, "oracle_asan_driver.c"),
+                    os.path.join(here, "..", "oracle", "bard_oracle.c"), "-lm"], check=True)
+    r = subprocess.run([exe], capture_output=True, text=True, env=dict(os.environ, ASAN_OPTIONS="detect_leaks=1"))
+    assert r.returncode == 0, r.stdout + r.stderr
+    assert "rc 0" in r.stdout and "ERROR" not in r.stderr and "runtime error" not in r.stderr

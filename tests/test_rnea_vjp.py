@@ -128,3 +128,165 @@ def test_vjp_is_the_transpose_of_the_regressor():
     lhs = float((g * dth).sum())
     rhs = float((dtau * o.rnea_params(q, qd, qdd, dth)).sum())
     assert abs(lhs - rhs) <= 1e-10 * max(1.0, abs(rhs))
+
+
+# ------------------------------------------------------------------------------------------- GPU
+torch = pytest.importorskip("torch")
+TOL = 1e-3        # as for RNEA itself (north_star): per element |g - ref| / max(1, |ref|)
+
+
+def nerr(x, ref):
+    return float(np.max(np.abs(np.asarray(x, np.float64) - ref) / np.maximum(1.0, np.abs(ref)))) if ref.size else 0.0
+
+
+def gpu_vjp(m, q, qd, qdd, dtau, repeat=1):
+    dev = torch.device("cuda:0")
+    B = q.shape[1]
+    t = [torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).to(dev) for a in (q, qd, qdd, dtau)]
+    ws = torch.full((max(1, m.rnea_vjp_workspace_floats(B)),), float("nan"), device=dev)
+    outs = []
+    for _ in range(repeat):
+        g = torch.full((m.nb, 10), float("nan"), device=dev)
+        m.rnea_vjp_params(B, *t, g, ws, torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        outs.append(g.cpu().numpy())
+    return outs if repeat > 1 else outs[0]
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("idx", range(8))
+@pytest.mark.parametrize("B", [1, 37, 1000, 4096 + 17])
+def test_gpu_vjp_matches_oracle(idx, B):
+    desc = _robots()[idx]
+    m = binding.Model(desc, device=0)
+    o = oracle.Oracle(desc)
+    np.testing.assert_allclose(m.inertial_params(), o.inertial_params(), rtol=0, atol=1e-14)
+    q, qd, qdd = W.sample_states(desc, B, seed=51 + idx)
+    dtau = np.random.default_rng(idx).normal(size=(desc.nv, B)).astype(np.float32)
+    g1, g2 = gpu_vjp(m, q, qd, qdd, dtau, repeat=2)
+    assert np.isfinite(g1).all()
+    assert np.array_equal(g1, g2)                                            # deterministic batch reduction
+    ref = o.rnea_vjp_params(*(a.astype(np.float64) for a in (q, qd, qdd, dtau)))
+    assert nerr(g1, ref) <= TOL
+
+
+@pytest.mark.gpu
+def test_gpu_vjp_full_size_and_adjoint_identity():
+    """Humanoid at B = 65 536 (bench size): against the oracle's definition (240 RNEA evaluations per environment on the
+    host cores), and the adjoint identity dparams . dtheta = sum dtau . tau(dtheta) with tau(dtheta) from the GPU's own
+    bard_rnea after bard_model_set_inertial_params(dtheta) -- the VJP is the transpose of what bard_rnea computes."""
+    desc = W.config_robot(3)
+    B = 65536
+    m = binding.Model(desc, device=0)
+    o = oracle.Oracle(desc)
+    q, qd, qdd = W.config_states(3, B)
+    rng = np.random.default_rng(8)
+    dtau = rng.normal(size=(desc.nv, B)).astype(np.float32)
+    g = gpu_vjp(m, q, qd, qdd, dtau)
+    ref = o.rnea_vjp_params(*(a.astype(np.float64) for a in (q, qd, qdd, dtau)))
+    assert nerr(g, ref) <= TOL
+    dth = o.inertial_params() * (1.0 + 0.3 * rng.normal(size=(desc.nb, 10)))   # a direction of physical magnitude
+    m.set_inertial_params(dth)
+    dev = torch.device("cuda:0")
+    tq, tqd, tqdd = (torch.from_numpy(a).to(dev) for a in (q, qd, qdd))
+    tau = torch.empty((desc.nv, B), device=dev)
+    m.rnea(B, tq, tqd, tqdd, tau, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    rhs = float((tau.double().cpu().numpy() * dtau.astype(np.float64)).sum())
+    lhs = float((g.astype(np.float64) * dth).sum())
+    scale = float(np.abs(g.astype(np.float64) * dth).sum())
+    assert abs(lhs - rhs) <= 1e-4 * scale
+
+
+@pytest.mark.gpu
+def test_set_inertial_params_reaches_every_kernel_family():
+    """After bard_model_set_inertial_params the team kernels read the new constants at once and the generated RNEA / CRBA
+    are dropped (they had the old parameters as literals) until the model is specialised again."""
+    desc = W.config_robot(1)
+    m = binding.Model(desc, device=0)
+    m.set_option("spec_min_b", 0)
+    m.specialize(("rnea", "crba"))
+    rng = np.random.default_rng(2)
+    new = copy.deepcopy(desc)
+    new.mass = desc.mass * rng.uniform(0.5, 2.0, size=desc.nb)
+    new.com = desc.com + rng.uniform(-0.02, 0.02, size=desc.com.shape)
+    m.set_inertial_params(theta_of(new))
+    with pytest.raises(binding.BardError):
+        m.specialized_source("rnea")
+    o = oracle.Oracle(new)
+    B = 500
+    q, qd, qdd = W.config_states(1, B)
+    dev = torch.device("cuda:0")
+    tq, tqd, tqdd = (torch.from_numpy(a).to(dev) for a in (q, qd, qdd))
+    q64, qd64, qdd64 = (a.astype(np.float64) for a in (q, qd, qdd))
+    for spec in (False, True):
+        if spec:
+            m.specialize(("rnea", "crba"))
+        tau = torch.full((desc.nv, B), float("nan"), device=dev)
+        M = torch.full((desc.nv, desc.nv, B), float("nan"), device=dev)
+        s = torch.cuda.current_stream().cuda_stream
+        m.rnea(B, tq, tqd, tqdd, tau, s)
+        m.crba(B, tq, M, s)
+        torch.cuda.synchronize()
+        assert nerr(tau.cpu().numpy(), o.rnea(q64, qd64, qdd64)) <= 1e-3
+        assert nerr(M.cpu().numpy(), o.crba(q64)) <= 1e-3
+
+
+@pytest.mark.gpu
+def test_synthetic_system_identification_of_link_masses():
+    """The paper's experiment (Table 2) on a stand-in: its KUKA iiwa data and Pinocchio ground truth are
+    not available, so config 0 (7-DOF chain) plays the arm, the "measured" torques are our own bard_rnea at the true
+    masses with 5 % multiplicative noise, and L-BFGS recovers the seven link masses from a 2x-off start through
+    loss = 1/2B sum |tau(m) - tau_meas|^2, gradient = bard_rnea_vjp_params chained to the masses (COM and inertia about
+    the COM held fixed).  The loss is quadratic in m, so the optimum is also available in closed form from the oracle's
+    regressor: L-BFGS through the GPU gradient must land on it."""
+    from scipy.optimize import minimize
+    desc = W.config_robot(0)
+    B = 4096
+    dev = torch.device("cuda:0")
+    m = binding.Model(desc, device=0)
+    q, qd, qdd = W.sample_states(desc, B, seed=77)
+    tq, tqd, tqdd = (torch.from_numpy(a).to(dev) for a in (q, qd, qdd))
+    s = torch.cuda.current_stream().cuda_stream
+    tau = torch.empty((desc.nv, B), device=dev)
+    m.rnea(B, tq, tqd, tqdd, tau, s)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(0)
+    meas = tau * torch.from_numpy((1 + 0.05 * rng.normal(size=(desc.nv, B))).astype(np.float32)).to(dev)
+    ws = torch.empty(m.rnea_vjp_workspace_floats(B), device=dev)
+    g = torch.empty((desc.nb, 10), device=dev)
+
+    def theta(mass):
+        d = copy.deepcopy(desc)
+        d.mass = np.asarray(mass, float)
+        return theta_of(d)
+
+    c = desc.com
+    dth_dm = np.zeros((desc.nb, 10))                                           # d theta_i / d m_i with c, Ic fixed
+    dth_dm[:, 0] = 1.0
+    dth_dm[:, 1:4] = c
+    c2 = (c * c).sum(1)
+    dth_dm[:, 4], dth_dm[:, 7], dth_dm[:, 9] = c2 - c[:, 0] ** 2, c2 - c[:, 1] ** 2, c2 - c[:, 2] ** 2
+    dth_dm[:, 5], dth_dm[:, 6], dth_dm[:, 8] = -c[:, 0] * c[:, 1], -c[:, 0] * c[:, 2], -c[:, 1] * c[:, 2]
+
+    def loss_and_grad(mass):
+        m.set_inertial_params(theta(mass))
+        m.rnea(B, tq, tqd, tqdd, tau, s)
+        r = (tau - meas) / B
+        m.rnea_vjp_params(B, tq, tqd, tqdd, r, g, ws, s)
+        torch.cuda.synchronize()
+        loss = 0.5 * B * float((r.double() ** 2).sum())
+        return loss, (g.double().cpu().numpy() * dth_dm).sum(1)
+
+    m0 = desc.mass * np.where(np.arange(desc.nb) % 2 == 0, 2.0, 0.5)
+    l0, _ = loss_and_grad(m0)
+    res = minimize(loss_and_grad, m0, jac=True, method="L-BFGS-B", options={"maxiter": 200, "ftol": 1e-14, "gtol": 1e-9})
+    # closed-form optimum from the oracle (fp64 regressor in the masses)
+    o = oracle.Oracle(desc)
+    q64, qd64, qdd64 = (a.astype(np.float64) for a in (q, qd, qdd))
+    t0 = o.rnea_params(q64, qd64, qdd64, theta(np.zeros(desc.nb)))
+    Y = np.stack([(o.rnea_params(q64, qd64, qdd64, theta(np.eye(desc.nb)[i])) - t0).ravel() for i in range(desc.nb)], 1)
+    best = np.linalg.lstsq(Y, (meas.double().cpu().numpy() - t0).ravel(), rcond=None)[0]
+    assert res.fun < 0.05 * l0
+    np.testing.assert_allclose(res.x, best, rtol=5e-3, atol=1e-3)               # the optimiser reached the least-squares optimum
+    assert np.max(np.abs(res.x - desc.mass) / desc.mass) < 0.15                 # and the masses are recovered (5 % torque noise)
