@@ -190,6 +190,28 @@ size_t      bard_aba_workspace_floats(const bard_model* m, int64_t B);
 bard_status bard_aba(const bard_model* m, int64_t B, const float* q, const float* qd, const float* tau, float* qdd,
                      float* workspace, bard_stream stream);
 
+/* Precision and layout variants of the four operators.
+ *   dtype : BARD_F32 (default) or BARD_F64 -- the whole recursion in double, model constants as the builder's unrounded
+ *           doubles: the instantiation that reproduces the paper's fp64 agreement table (Table 1)
+ *           against the fp64 oracle (<= 1e-11 on the BASELINE robots).
+ *   layout: BARD_LAYOUT_SOA (default: [rows][B], batch fastest) or BARD_LAYOUT_AOS -- the paper's batch-first layout
+ *           (PAPER.md:103): q (B, nq), qd / qdd / tau (B, nv), pose (B, nb, 12), J (B, nframes, 6, nv), M (B, nv, nv),
+ *           contiguous, so PyTorch callers pass their (B, n) tensors without a transpose.
+ * bard_model_specialize_variant generates and compiles the operators in `ops` (BARD_OP_FK | JACOBIAN | RNEA | CRBA) for
+ * that (dtype, layout) with NVRTC, as bard_model_specialize does; the _v calls launch them at every batch size (one
+ * launch, asynchronous; pointers are device pointers to float or double according to dtype).  (BARD_F32,
+ * BARD_LAYOUT_SOA) is the plain operator call.  Without the variant kernel: BARD_ERR_UNSUPPORTED.
+ * bard_model_set_frames / set_inertial_params drop the variants that depend on them, like the plain kernels. */
+enum { BARD_F32 = 0, BARD_F64 = 1 };
+enum { BARD_LAYOUT_SOA = 0, BARD_LAYOUT_AOS = 1 };
+bard_status bard_model_specialize_variant(bard_model* m, uint32_t ops, int dtype, int layout);
+bard_status bard_model_variant_source(const bard_model* m, uint32_t op, int dtype, int layout, char* host_dst, size_t cap, size_t* need);
+bard_status bard_fk_v      (const bard_model* m, int dtype, int layout, int64_t B, const void* q, void* pose, bard_stream stream);
+bard_status bard_jacobian_v(const bard_model* m, int dtype, int layout, int64_t B, const void* q, void* J, bard_stream stream);
+bard_status bard_rnea_v    (const bard_model* m, int dtype, int layout, int64_t B, const void* q, const void* qd, const void* qdd,
+                            void* tau, bard_stream stream);
+bard_status bard_crba_v    (const bard_model* m, int dtype, int layout, int64_t B, const void* q, void* M, bard_stream stream);
+
 /* Reverse-mode derivative of RNEA with respect to the inertial parameters (the paper's
  * differentiable "functional mode", and its use: link masses identified through RNEA).
  * theta[nb][10] per link: m, h = m c (3), Io = Ic + m [c]x [c]x^T (xx,xy,xz,yy,yz,zz about the BODY ORIGIN, body axes);

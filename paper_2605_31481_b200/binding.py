@@ -21,12 +21,15 @@ BARD_OK = 0
 STATUS = {0: "BARD_OK", 1: "BARD_ERR_INVALID_ARG", 2: "BARD_ERR_TOPOLOGY", 3: "BARD_ERR_UNSUPPORTED",
           4: "BARD_ERR_ALLOC", 5: "BARD_ERR_CUDA"}
 OPS = {"fk": 1, "jacobian": 2, "rnea": 4, "crba": 8, "fused": 16, "aba": 32, "rnea_roles": 64, "crba_roles": 128}
+DTYPES = {"f32": 0, "f64": 1}
+LAYOUTS = {"soa": 0, "aos": 1}
 TABLES = {"LEVEL_PTR": (0, np.int32), "LEVEL_BODY": (1, np.int32), "BODY_LEVEL": (2, np.int32),
           "PARENT_SLOT": (3, np.int32), "Q_OFF": (4, np.int32), "V_OFF": (5, np.int32), "DOF_BODY": (6, np.int32),
           "ANC_MASK": (7, np.uint64), "RODRIGUES": (8, np.float32)}
 EXPORTS = ["bard_model_create", "bard_model_destroy", "bard_model_dims", "bard_model_get_table",
            "bard_model_set_frames", "bard_model_set_option", "bard_model_get_option", "bard_model_specialize", "bard_model_specialized_source", "bard_fk", "bard_jacobian", "bard_rnea", "bard_crba", "bard_step", "bard_euler_step", "bard_aba", "bard_aba_workspace_floats", "bard_rnea_vjp_params", "bard_rnea_vjp_workspace_floats",
-           "bard_model_inertial_params", "bard_model_set_inertial_params",
+           "bard_model_inertial_params", "bard_model_set_inertial_params", "bard_model_specialize_variant", "bard_model_variant_source",
+           "bard_fk_v", "bard_jacobian_v", "bard_rnea_v", "bard_crba_v",
            "bard_status_string", "bard_last_error", "bard_launch_count"]
 
 
@@ -79,6 +82,12 @@ def lib():
         L.bard_rnea_vjp_params.argtypes = [vp, i64, fp, fp, fp, fp, fp, fp, vp]
         L.bard_model_inertial_params.argtypes = [vp, C.POINTER(C.c_double)]
         L.bard_model_set_inertial_params.argtypes = [vp, C.POINTER(C.c_double)]
+        L.bard_model_specialize_variant.argtypes = [vp, C.c_uint32, C.c_int, C.c_int]
+        L.bard_model_variant_source.argtypes = [vp, C.c_uint32, C.c_int, C.c_int, C.c_char_p, C.c_size_t, C.POINTER(C.c_size_t)]
+        L.bard_fk_v.argtypes = [vp, C.c_int, C.c_int, i64, fp, fp, vp]
+        L.bard_jacobian_v.argtypes = [vp, C.c_int, C.c_int, i64, fp, fp, vp]
+        L.bard_rnea_v.argtypes = [vp, C.c_int, C.c_int, i64, fp, fp, fp, fp, vp]
+        L.bard_crba_v.argtypes = [vp, C.c_int, C.c_int, i64, fp, fp, vp]
         L.bard_status_string.argtypes = [C.c_int]
         L.bard_status_string.restype = C.c_char_p
         L.bard_last_error.restype = C.c_char_p
@@ -223,6 +232,32 @@ class Model:
     def aba(self, B, q, qd, tau, qdd, workspace, stream=0):
         """Forward dynamics qdd = M^-1 (tau - C) (``bard_aba``); needs ``specialize(("aba",))`` first."""
         _check(lib().bard_aba(self._h, int(B), _ptr(q), _ptr(qd), _ptr(tau), _ptr(qdd), _ptr(workspace), stream or None))
+
+    # ---- dtype / layout variants (``bard_*_v``): dtype "f32" | "f64", layout "soa" | "aos" (batch-first, the paper's)
+    def specialize_variant(self, ops, dtype="f32", layout="soa"):
+        mask = 0
+        for o in ops:
+            mask |= OPS[o]
+        _check(lib().bard_model_specialize_variant(self._h, mask, DTYPES[dtype], LAYOUTS[layout]))
+
+    def variant_source(self, op: str, dtype="f32", layout="soa") -> str:
+        need = C.c_size_t()
+        lib().bard_model_variant_source(self._h, OPS[op], DTYPES[dtype], LAYOUTS[layout], None, 0, C.byref(need))
+        buf = C.create_string_buffer(max(need.value, 1))
+        _check(lib().bard_model_variant_source(self._h, OPS[op], DTYPES[dtype], LAYOUTS[layout], buf, need.value, C.byref(need)))
+        return buf.value.decode()
+
+    def fk_v(self, dtype, layout, B, q, pose, stream=0):
+        _check(lib().bard_fk_v(self._h, DTYPES[dtype], LAYOUTS[layout], int(B), _ptr(q), _ptr(pose), stream or None))
+
+    def jacobian_v(self, dtype, layout, B, q, J, stream=0):
+        _check(lib().bard_jacobian_v(self._h, DTYPES[dtype], LAYOUTS[layout], int(B), _ptr(q), _ptr(J), stream or None))
+
+    def rnea_v(self, dtype, layout, B, q, qd, qdd, tau, stream=0):
+        _check(lib().bard_rnea_v(self._h, DTYPES[dtype], LAYOUTS[layout], int(B), _ptr(q), _ptr(qd), _ptr(qdd), _ptr(tau), stream or None))
+
+    def crba_v(self, dtype, layout, B, q, M, stream=0):
+        _check(lib().bard_crba_v(self._h, DTYPES[dtype], LAYOUTS[layout], int(B), _ptr(q), _ptr(M), stream or None))
 
     def rnea_vjp_workspace_floats(self, B) -> int:
         return int(lib().bard_rnea_vjp_workspace_floats(self._h, int(B)))

@@ -298,6 +298,55 @@ bard_status bard_aba(const bard_model* bm, int64_t B, const float* q, const floa
   return bard::launch_aba(bm->m, B, q, qd, tau, qdd, workspace, stream);
 }
 
+bard_status bard_model_specialize_variant(bard_model* bm, uint32_t ops, int dtype, int layout) {
+  if (!bm) { set_error("bard_model_specialize_variant: model is NULL"); return BARD_ERR_INVALID_ARG; }
+  return bard::specialize_variant(bm->m, ops, dtype, layout);
+}
+
+bard_status bard_model_variant_source(const bard_model* bm, uint32_t op, int dtype, int layout, char* host_dst, size_t cap, size_t* need) {
+  if (!bm) { set_error("bard_model_variant_source: model is NULL"); return BARD_ERR_INVALID_ARG; }
+  const std::string* src = bard::variant_source(bm->m, op, dtype, layout);
+  if (!src) { set_error("bard_model_variant_source: operator variant not specialised"); return BARD_ERR_INVALID_ARG; }
+  if (need) *need = src->size() + 1;
+  if (cap < src->size() + 1 || !host_dst) { set_error("bard_model_variant_source: destination too small"); return BARD_ERR_INVALID_ARG; }
+  std::memcpy(host_dst, src->c_str(), src->size() + 1);
+  return BARD_OK;
+}
+
+// the _v calls: dtype / layout variants of the four operators.  (F32, SoA) is the plain call.
+static bard_status variant_call(const char* fn, const bard_model* bm, uint32_t op, int dtype, int layout, int64_t B, const void* q,
+                                const void* qd, const void* qdd, void* pose, void* J, void* tau, void* Mo, bard_stream stream) {
+  if (!bm) { set_error(std::string(fn) + ": model is NULL"); return BARD_ERR_INVALID_ARG; }
+  if (dtype < 0 || dtype > 1 || layout < 0 || layout > 1) { set_error(std::string(fn) + ": unknown dtype / layout"); return BARD_ERR_INVALID_ARG; }
+  const bard::Model& m = bm->m;
+  const bool empty = (op != BARD_OP_FK && m.nv == 0) || (op == BARD_OP_JACOBIAN && m.nframes == 0);
+  void* out = op == BARD_OP_FK ? pose : op == BARD_OP_JACOBIAN ? J : op == BARD_OP_RNEA ? tau : Mo;
+  const void* dummy = bm;
+  bard_status s = check_call(fn, bm, B, (m.nq == 0 || empty) ? dummy : q, (op == BARD_OP_RNEA && !empty) ? qd : dummy,
+                             (op == BARD_OP_RNEA && !empty) ? qdd : dummy, empty ? dummy : out);
+  if (s != BARD_OK || B == 0 || empty) return s;
+  bard::DeviceGuard guard(m.device);
+  return bard::launch_variant(m, op, dtype, layout, B, q, qd, qdd, pose, J, tau, Mo, stream);
+}
+
+bard_status bard_fk_v(const bard_model* bm, int dtype, int layout, int64_t B, const void* q, void* pose, bard_stream stream) {
+  if (dtype == BARD_F32 && layout == BARD_LAYOUT_SOA) return bard_fk(bm, B, (const float*)q, (float*)pose, stream);
+  return variant_call("bard_fk_v", bm, BARD_OP_FK, dtype, layout, B, q, nullptr, nullptr, pose, nullptr, nullptr, nullptr, stream);
+}
+bard_status bard_jacobian_v(const bard_model* bm, int dtype, int layout, int64_t B, const void* q, void* J, bard_stream stream) {
+  if (dtype == BARD_F32 && layout == BARD_LAYOUT_SOA) return bard_jacobian(bm, B, (const float*)q, (float*)J, stream);
+  return variant_call("bard_jacobian_v", bm, BARD_OP_JACOBIAN, dtype, layout, B, q, nullptr, nullptr, nullptr, J, nullptr, nullptr, stream);
+}
+bard_status bard_rnea_v(const bard_model* bm, int dtype, int layout, int64_t B, const void* q, const void* qd, const void* qdd, void* tau,
+                        bard_stream stream) {
+  if (dtype == BARD_F32 && layout == BARD_LAYOUT_SOA) return bard_rnea(bm, B, (const float*)q, (const float*)qd, (const float*)qdd, (float*)tau, stream);
+  return variant_call("bard_rnea_v", bm, BARD_OP_RNEA, dtype, layout, B, q, qd, qdd, nullptr, nullptr, tau, nullptr, stream);
+}
+bard_status bard_crba_v(const bard_model* bm, int dtype, int layout, int64_t B, const void* q, void* M, bard_stream stream) {
+  if (dtype == BARD_F32 && layout == BARD_LAYOUT_SOA) return bard_crba(bm, B, (const float*)q, (float*)M, stream);
+  return variant_call("bard_crba_v", bm, BARD_OP_CRBA, dtype, layout, B, q, nullptr, nullptr, nullptr, nullptr, nullptr, M, stream);
+}
+
 size_t bard_rnea_vjp_workspace_floats(const bard_model* bm, int64_t B) {
   return (bm && B > 0) ? bard::rnea_vjp_workspace_floats(bm->m, B) : 0;
 }

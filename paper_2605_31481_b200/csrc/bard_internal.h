@@ -194,6 +194,10 @@ void free_specialized(Specialized* s);
 const std::string* specialized_source(const Model& M, uint32_t op);
 bool launch_specialized(const Model& M, uint32_t op, int64_t B, const float* q, const float* qd, const float* qdd, float* pose,
                         float* J, float* tau, float* Mo, void* stream, bard_status& st);
+bard_status specialize_variant(Model& M, uint32_t ops, int dtype, int layout);
+const std::string* variant_source(const Model& M, uint32_t op, int dtype, int layout);
+bard_status launch_variant(const Model& M, uint32_t op, int dtype, int layout, int64_t B, const void* q, const void* qd, const void* qdd,
+                           void* pose, void* J, void* tau, void* Mo, void* stream);
 void drop_specialized_jacobian(Model& M);
 void drop_specialized_dynamics(Model& M);      // kernels with the inertial parameters folded in as literals
 
