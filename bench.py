@@ -1,18 +1,26 @@
 #!/usr/bin/env python
 """bench.py -- one JSON line for the batched rigid-body hot path (FK, Jacobian, RNEA, CRBA) on B200.
 
-A "step" is one pass of the whole hot path over one batch of synthetic states: bard_fk, bard_jacobian,
-bard_rnea and bard_crba (four kernel launches through the C ABI) on B environments.  One "env-eval" is all
-four operators evaluated for one environment.  Default workload: config 3 (23-DOF humanoid) at B = 65 536,
-the point of BASELINE.json's sweep (config 4) from which north_star's roofline target applies.
+A "step" is one pass of the whole hot path over one batch of synthetic states: ``bard_step`` = bard_fk, bard_jacobian,
+bard_rnea and bard_crba of one (q, qd, qdd) batch through the C ABI.  One "env-eval" is all four operators evaluated
+for one environment.  Headline workload: config 3 (23-DOF humanoid) at B = 65 536, the point of BASELINE.json's sweep
+(config 4) from which north_star's roofline target applies.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0..3] [--B n] [--impl ours|reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0..3] [--B n] [--impl ours|reference] [--quick]
 
-Multi-GPU (N > 1, under torch.distributed.run): the batch axis shards, every rank evaluates its own B
-environments with a replicated model and no data-path collective -> "scaling": "weak".
+Besides the headline the default run (rank 0, one GPU) reports, compactly:
+  * ``matrix``: every operator and bard_step on configs 0-3 at B = 4096 and 65 536 (BASELINE.json's metric);
+  * ``sweep``: BASELINE.json config 4 -- humanoid and chain-7 at B = 1024 ... 1 048 576: env-evals/s, achieved HBM GB/s
+    and FP32 TFLOP/s against the B200 peaks, and the oracle's time on the host cores per B;
+  * ``aba`` (with its roofline), ``rnea_vjp``, ``variants`` (fp64 / AoS), ``config2_rollout``, ``specialize_s``.
+Per-operator times are device times of a back-to-back train of launches over rotating buffer sets (> L2 in total)
+replayed from a CUDA graph, so that a kernel shorter than the host's launch rate is timed as a kernel.
 
-``--impl reference`` times the fp64 CPU oracle (oracle/, test infrastructure) on a bounded sample of the
-same workload on the host cores; rank 0 only.
+Multi-GPU (N > 1, under torch.distributed.run): the batch axis shards, every rank evaluates its own B environments with
+a replicated model and no data-path collective -> "scaling": "weak"; headline and e2e only.
+
+``--impl reference`` times the fp64 CPU oracle (oracle/, test infrastructure) on a bounded sample of the same workload on
+the host cores; rank 0 only.
 """
 from __future__ import annotations
 
@@ -29,14 +37,16 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+from paper_2605_31481_b200 import dist as D                 # noqa: E402
 from paper_2605_31481_b200 import roofline as RL            # noqa: E402
 from paper_2605_31481_b200 import workloads as W            # noqa: E402
 
 OPS = ("fk", "jacobian", "rnea", "crba")
-SPEC_OPS = ("fk", "jacobian", "rnea", "crba", "fused")   # "fused": the one-kernel bard_step (built for small robots)
+SPEC_OPS = ("fk", "jacobian", "rnea", "crba", "fused")   # "fused": the one-kernel forms of bard_step
 METRIC = "env_evals_per_s (FK + Jacobian + RNEA + CRBA per environment)"
 UNIT = "env-evals/s"
 L2_BYTES = 126 * 1024 * 1024
+SWEEP_B = (1024, 4096, 16384, 65536, 262144, 1048576)
 
 
 def parse():
@@ -47,7 +57,9 @@ def parse():
     ap.add_argument("--config", type=int, default=3, choices=[0, 1, 2, 3])
     ap.add_argument("--B", type=int, default=65536)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--sweep", action="store_true", help="also time every operator over config 4's batch sweep")
+    ap.add_argument("--quick", action="store_true", help="headline, e2e and cpu_baseline only (no matrix / sweep / extras)")
+    ap.add_argument("--no-sweep", action="store_true", help="skip BASELINE config 4's batch sweep")
+    ap.add_argument("--no-matrix", action="store_true", help="skip configs 0-3 x B in {4096, 65536}")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-rollout", action="store_true", help="skip the config-2 24-step rollout section")
     ap.add_argument("--no-specialize", action="store_true",
@@ -60,36 +72,48 @@ def workload_name(cfg, B):
     return f"config{cfg}:{W.CONFIG_NAMES[cfg]} B={B} (sweep point of config 4)"
 
 
+def sig(x, n=4):
+    """Round to n significant digits (keeps the JSON line compact)."""
+    if x is None or isinstance(x, (str, bool, int)):
+        return x
+    if isinstance(x, dict):
+        return {k: sig(v, n) for k, v in x.items()}
+    if isinstance(x, (list, tuple)):
+        return [sig(v, n) for v in x]
+    x = float(x)
+    return x if x == 0 or not np.isfinite(x) else float(f"{x:.{n}g}")
+
+
 # --------------------------------------------------------------------------------------- oracle timing
+def oracle_pass_seconds(o, q, qd, qdd):
+    t0 = time.perf_counter()
+    o.fk(q)
+    o.jacobian(q)
+    o.rnea(q, qd, qdd)
+    o.crba(q)
+    return time.perf_counter() - t0
+
+
 def time_oracle(desc, cfg, seconds):
-    """The fp64 oracle as it stands, all four operators, OpenMP over environments on the host cores, on a
-    bounded sample of the workload's states (same seeded distributions).  Returns env-evals/s and details."""
+    """The fp64 oracle as it stands, all four operators, OpenMP over environments on the host cores, on a bounded sample
+    of the workload's states (same seeded distributions).  Returns the cpu_baseline object."""
     import oracle
     o = oracle.Oracle(desc)
     cores = os.cpu_count() or 1
     oracle.set_threads(cores)
     used = oracle.get_threads()
-
-    def one_pass(q, qd, qdd):
-        t0 = time.perf_counter()
-        o.fk(q)
-        o.jacobian(q)
-        o.rnea(q, qd, qdd)
-        o.crba(q)
-        return time.perf_counter() - t0
-
     n = 16384
     q, qd, qdd = (a.astype(np.float64) for a in W.config_states(cfg, n))
-    one_pass(q, qd, qdd)                                  # warm pass (page-in, thread pool)
-    t = one_pass(q, qd, qdd)
+    oracle_pass_seconds(o, q, qd, qdd)                    # warm pass (page-in, thread pool)
+    t = oracle_pass_seconds(o, q, qd, qdd)
     passes = int(max(3, min(200, np.ceil(seconds / max(t, 1e-6)))))
     t0 = time.perf_counter()
     for _ in range(passes):
-        one_pass(q, qd, qdd)
+        oracle_pass_seconds(o, q, qd, qdd)
     total = time.perf_counter() - t0
     return {"value": n * passes / total, "unit": UNIT, "cores": used, "kind": "oracle",
             "sample": f"{passes} passes over {n} environments of the workload's seeded state distribution, all four "
-                      f"operators, fp64, OpenMP over environments ({total:.1f} s of CPU work)"}, n, total
+                      f"operators, fp64, OpenMP over environments ({total:.1f} s of CPU work)"}
 
 
 def run_reference(args):
@@ -100,29 +124,24 @@ def run_reference(args):
     import oracle
     o = oracle.Oracle(desc)
     oracle.set_threads(os.cpu_count() or 1)
-    n = 8192                                             # bounded sample per step
+    steps, warm = max(1, args.steps), max(0, args.warmup)
+    # a bounded sample of the workload per step, sized so that the whole run stays within about a minute of CPU work
+    n = int(min(8192, max(256, 8192 * 1500 // max(1, steps + warm))))
     q, qd, qdd = (a.astype(np.float64) for a in W.config_states(args.config, n))
-
-    def step():
-        o.fk(q); o.jacobian(q); o.rnea(q, qd, qdd); o.crba(q)
-
-    steps = min(args.steps, 20)
-    warm = min(args.warmup, 3)
     for _ in range(warm):
-        step()
+        oracle_pass_seconds(o, q, qd, qdd)
     t0 = time.perf_counter()
     for _ in range(steps):
-        step()
+        oracle_pass_seconds(o, q, qd, qdd)
     dt = time.perf_counter() - t0
     val = n * steps / dt
     line = {
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
         "warmup": warm, "ms_per_step": 1e3 * dt / steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_name(args.config, args.B),
-                   "note": f"oracle timed on a bounded sample of {n} environments per step (host cores)"},
+        "config": {"workload": workload_name(args.config, args.B)},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": oracle.get_threads(), "kind": "oracle",
-                         "sample": f"{n} environments per step x {steps} steps"},
+                         "sample": f"the fp64 oracle on the host cores, a bounded sample of {n} environments of the workload per step x {steps} steps"},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -178,9 +197,11 @@ class Clocks(threading.Thread):
 class BufferSet:
     """One set of device inputs and outputs (SoA, batch last) for B environments."""
 
-    def __init__(self, torch, m, desc, cfg, B, seed_step, dev):
-        q, qd, qdd = W.sample_states(desc, B, seed=2000 + cfg + 100 * seed_step)
-        self.q, self.qd, self.qdd = (torch.from_numpy(a).to(dev) for a in (q, qd, qdd))
+    def __init__(self, torch, m, ins, shift, dev):
+        # the first set holds the seeded states; the others are the same states rolled along the batch axis on the
+        # device (same distribution, other addresses and another environment per lane) -- no host RNG per set
+        self.q, self.qd, self.qdd = (t if shift == 0 else torch.roll(t, shifts=shift, dims=1) for t in ins)
+        B = self.q.shape[1]
         self.pose = torch.empty((m.nb, 12, B), device=dev)
         self.J = torch.empty((m.nframes, 6, m.nv, B), device=dev)
         self.tau = torch.empty((m.nv, B), device=dev)
@@ -197,39 +218,32 @@ def op_call(m, op, s, B, stream):
         m.jacobian(B, s.q, s.J, stream)
     elif op == "rnea":
         m.rnea(B, s.q, s.qd, s.qdd, s.tau, stream)
-    else:
+    elif op == "crba":
         m.crba(B, s.q, s.M, stream)
+    else:
+        m.step(B, s.q, s.qd, s.qdd, s.pose, s.J, s.tau, s.M, stream)
 
 
 def make_sets(torch, m, desc, cfg, B, dev, min_sets=3, cap_bytes=48 << 30):
-    first = BufferSet(torch, m, desc, cfg, B, 0, dev)
+    ins = [torch.from_numpy(a).to(dev) for a in W.sample_states(desc, B, seed=2000 + cfg)]
+    first = BufferSet(torch, m, ins, 0, dev)
     per = first.nbytes()
     n = max(min_sets, -(-3 * L2_BYTES // per))           # rotating sets: total >= 3 x L2
-    n = max(1, min(n, cap_bytes // per))
-    return [first] + [BufferSet(torch, m, desc, cfg, B, i, dev) for i in range(1, n)], per
+    n = max(1, min(n, cap_bytes // per, 64))
+    return [first] + [BufferSet(torch, m, ins, 17 + 31 * i, dev) for i in range(1, n)], per
 
 
-def time_op_train(torch, m, op, sets, B, stream, launches, warm=5):
-    """Average duration of one launch of `op`, back to back over rotating buffer sets, CUDA events on `stream`."""
-    for i in range(warm):
-        op_call(m, op, sets[i % len(sets)], B, stream)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    torch.cuda.synchronize()
-    e0.record()
-    for i in range(launches):
-        op_call(m, op, sets[i % len(sets)], B, stream)
-    e1.record()
-    torch.cuda.synchronize()
-    return e0.elapsed_time(e1) * 1e-3 / launches
-
-
-def time_op_graph(torch, m, op, sets, B, launches=64, replays=10):
-    """Same train captured once into a CUDA graph and replayed: device-side time per launch without the host's
-    per-call cost (at B = 4096 a launch through ctypes costs more than the kernel)."""
+def time_graph(torch, m, op, sets, B, launches=None, replays=None):
+    """Device time per launch of a back-to-back train of `op` over the rotating buffer sets, captured once into a CUDA
+    graph and replayed (no host launch cost inside the timed region): (seconds per launch, launches per replay)."""
+    if launches is None:
+        launches = max(len(sets), 64 if B <= 65536 else 2 * len(sets))
+    if replays is None:
+        replays = 10 if B <= 65536 else 4
     side = torch.cuda.Stream()
     side.wait_stream(torch.cuda.current_stream())
     with torch.cuda.stream(side):
-        for i in range(4):
+        for i in range(min(4, launches)):
             op_call(m, op, sets[i % len(sets)], B, side.cuda_stream)
     torch.cuda.current_stream().wait_stream(side)
     torch.cuda.synchronize()
@@ -248,21 +262,47 @@ def time_op_graph(torch, m, op, sets, B, launches=64, replays=10):
     return e0.elapsed_time(e1) * 1e-3 / (launches * replays)
 
 
-def rollout_config2(torch, binding, dev, specialize=True, steps=24, dt=0.005, replays=10):
+def time_train(torch, m, op, sets, B, stream, launches, warm=5):
+    """Same train through plain host launches (one ctypes call each), CUDA events on `stream`."""
+    for i in range(warm):
+        op_call(m, op, sets[i % len(sets)], B, stream)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for i in range(launches):
+        op_call(m, op, sets[i % len(sets)], B, stream)
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) * 1e-3 / launches
+
+
+def op_report(desc, pk, op, sec, B):
+    r = RL.roofline(desc, pk)[op]
+    if r["bound"] == "hbm":
+        ach, peak, unit = r["bytes"] * B / sec / 1e9, pk["hbm_gbs"], "GB/s"
+    else:
+        ach, peak, unit = r["flop"] * B / sec / 1e12, pk["fp32_tflops"], "TFLOP/s"
+    return {"us": sec * 1e6, "env_evals_per_s": B / sec, "bound": r["bound"], "achieved": ach, "peak": peak,
+            "unit": unit, "frac": ach / peak, "bytes_per_env": r["bytes"], "flop_per_env": r["flop"],
+            "hbm_gbs": r["bytes"] * B / sec / 1e9, "fp32_tflops": r["flop"] * B / sec / 1e12}
+
+
+def short(r, keys=("us", "env_evals_per_s", "bound", "frac", "hbm_gbs", "fp32_tflops")):
+    return {k: r[k] for k in keys}
+
+
+def rollout_config2(torch, binding, m, desc, dev, steps=24, dt=0.005, replays=10):
     """BASELINE.json config 2: the 11-DOF spined quadruped, all four operators per simulated RL step (bard_step)
     over 24 consecutive steps, q advanced on the device by explicit Euler (bard_euler_step) from seeded random qdd.
     The 24-step loop is captured once into a CUDA graph and replayed; reported as env-steps/s."""
-    desc = W.config_robot(2)
-    m = binding.Model(desc, device=dev.index or 0)
-    if specialize:
-        m.specialize(SPEC_OPS)
     out = {}
     for B in (4096, 65536):
         q, qd, _ = W.sample_states(desc, B, seed=2002)
         q0, qd0 = torch.from_numpy(q).to(dev), torch.from_numpy(qd).to(dev)
         tq, tqd = q0.clone(), qd0.clone()
-        qdds = [torch.from_numpy(np.random.default_rng(2002 + 100 * (k + 1)).normal(size=(desc.nv, B)).astype(np.float32)).to(dev)
-                for k in range(steps)]
+        gen = torch.Generator(device=dev)
+        gen.manual_seed(2002)
+        qdds = [torch.randn((desc.nv, B), device=dev, generator=gen) for _ in range(steps)]
         outs = [torch.empty(sh, device=dev) for sh in ((m.nb, 12, B), (m.nframes, 6, m.nv, B), (m.nv, B), (m.nv, m.nv, B))]
 
         def loop(stream):
@@ -295,21 +335,9 @@ def rollout_config2(torch, binding, dev, specialize=True, steps=24, dt=0.005, re
             ms.append(e0.elapsed_time(e1))
         med = float(np.median(ms))
         out[f"B{B}"] = {"env_steps_per_s": B * steps / (med * 1e-3), "us_per_step": med * 1e3 / steps,
-                        "ms_per_24_steps": med, "launches_per_24_steps": int(per_loop), "finite": bool(torch.isfinite(outs[3]).all())}
-    m.close()
+                        "launches_per_24_steps": int(per_loop), "finite": bool(torch.isfinite(outs[3]).all())}
     out["note"] = "CUDA graph of 24 x (bard_step + bard_euler_step), dt 0.005, seeded qdd per step, median of 10 replays"
     return out
-
-
-def op_report(desc, pk, op, sec, B):
-    r = RL.roofline(desc, pk)[op]
-    if r["bound"] == "hbm":
-        ach, peak, unit = r["bytes"] * B / sec / 1e9, pk["hbm_gbs"], "GB/s"
-    else:
-        ach, peak, unit = r["flop"] * B / sec / 1e12, pk["fp32_tflops"], "TFLOP/s"
-    return {"us": sec * 1e6, "env_evals_per_s": B / sec, "bound": r["bound"], "achieved": ach, "peak": peak,
-            "unit": unit, "frac": ach / peak, "bytes_per_env": r["bytes"], "flop_per_env": r["flop"],
-            "hbm_gbs": r["bytes"] * B / sec / 1e9, "fp32_tflops": r["flop"] * B / sec / 1e12}
 
 
 def run_ours(args):
@@ -328,16 +356,34 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=dev)
 
     def barrier():
-        if world > 1:
-            dist.barrier()
+        D.barrier()
         torch.cuda.synchronize()
 
+    t_start = time.perf_counter()
+    extras = rank == 0 and world == 1 and not args.quick
     cfg, B, K, Wm = args.config, args.B, args.steps, max(args.warmup, 3)
-    desc = W.config_robot(cfg)
-    m = binding.Model(desc, device=local)
-    if not args.no_specialize:
-        m.specialize(SPEC_OPS)          # model-specialised (NVRTC) kernels for the operators that have a generator
-    pk = RL.measured_peaks(ROOT)
+    fp32_meas = None
+    try:
+        fp32_meas = binding.measure_fp32_peak(local)
+    except Exception:
+        pass
+    pk = RL.measured_peaks(ROOT, fp32_meas)
+
+    models, spec_s = {}, {}
+
+    def model(c):
+        """One model per config for the whole run; bard_model_specialize is timed (NVRTC: seconds per robot)."""
+        if c not in models:
+            d = W.config_robot(c)
+            mm = binding.Model(d, device=local)
+            if not args.no_specialize:
+                t0 = time.perf_counter()
+                mm.specialize(SPEC_OPS)
+                spec_s[W.CONFIG_NAMES[c]] = time.perf_counter() - t0
+            models[c] = (d, mm)
+        return models[c]
+
+    desc, m = model(cfg)
     sets, per_set = make_sets(torch, m, desc, cfg, B, dev)
     R = len(sets)
     stream = torch.cuda.current_stream().cuda_stream
@@ -346,23 +392,21 @@ def run_ours(args):
 
     def step(i, ev=None):
         s = sets[i % R]
-        if ev is None:      # the call a user makes: bard_step = all four operators of one batch (one fused kernel or four)
+        if ev is None:      # the call a user makes: bard_step = all four operators of one batch
             m.step(B, s.q, s.qd, s.qdd, s.pose, s.J, s.tau, s.M, stream)
             return
         for k, op in enumerate(OPS):
-            if ev is not None:
-                ev[k].record()
+            ev[k].record()
             op_call(m, op, s, B, stream)
-        if ev is not None:
-            ev[4].record()
+        ev[4].record()
 
     # ---- device-resident timed region: W warm-up steps, then exactly K steps
     for i in range(Wm):
         step(i)
     # The timed region is K uninstrumented steps between two events: an event record between two launches would
     # end the programmatic overlap of a kernel's prologue with the previous kernel's tail (PDL) and time the
-    # events themselves.  Per-operator durations come from a second, identical pass of K steps with an event
-    # before every launch (below); its step time is reported next to the headline as ms_per_step_instrumented.
+    # events themselves.  Per-operator durations come from a second pass of K steps, the four operators called one by
+    # one with an event before every launch; its step time is reported as ms_per_step_instrumented.
     e_beg, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     clocks.active.set()
@@ -374,8 +418,10 @@ def run_ours(args):
     barrier()
     clocks.active.clear()
     launches = binding.launch_count() - n0
-    elapsed_ms = e_beg.elapsed_time(e_end)
+    elapsed_ms = D.max_over_ranks(e_beg.elapsed_time(e_end), dev)
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(K)]
+    for i in range(Wm):
+        step(i, evs[0])
     barrier()
     clocks.active.set()
     for i in range(K):
@@ -383,57 +429,25 @@ def run_ours(args):
     barrier()
     clocks.active.clear()
     instrumented_ms = evs[0][0].elapsed_time(evs[-1][4])
-    t = torch.tensor([elapsed_ms], device=dev, dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    elapsed_ms = float(t.item())
     value = world * B * K / (elapsed_ms * 1e-3)
     op_sec = {op: float(np.mean([evs[i][k].elapsed_time(evs[i][k + 1]) for i in range(K)])) * 1e-3
               for k, op in enumerate(OPS)}
-    ops = {op: op_report(desc, pk, op, op_sec[op], B) for op in OPS}
+    ops = {}
     for op in OPS:
-        ops[op]["share_of_step"] = op_sec[op] / sum(op_sec.values())
-
-    # ---- per-operator back-to-back trains (no events between launches), same rotating buffers
+        r = op_report(desc, pk, op, op_sec[op], B)
+        ops[op] = {"in_step": short(r, ("us", "frac", "achieved")), "bound": r["bound"], "unit": r["unit"], "peak": r["peak"],
+                   "bytes_per_env": r["bytes_per_env"], "flop_per_env": r["flop_per_env"], "share_of_step": op_sec[op] / sum(op_sec.values())}
+    # ---- per-operator back-to-back trains, replayed from a CUDA graph (kernel time without host launch cost)
     clocks.active.set()
     for op in OPS:
-        sec = time_op_train(torch, m, op, sets, B, stream, launches=max(50, min(K, 500)))
-        ops[op]["train"] = {k: v for k, v in op_report(desc, pk, op, sec, B).items()
-                            if k in ("us", "env_evals_per_s", "achieved", "frac", "hbm_gbs", "fp32_tflops")}
-    # ---- the metric's other batch size: every operator at B = 4096 (latency-bound: roofline times <= 2.2 us)
-    small = {}
-    if B != 4096:
-        sets_s, _ = make_sets(torch, m, desc, cfg, 4096, dev, min_sets=8, cap_bytes=4 << 30)
-        for op in OPS:
-            sec = time_op_train(torch, m, op, sets_s, 4096, stream, launches=200)
-            r = op_report(desc, pk, op, sec, 4096)
-            small[op] = {k: r[k] for k in ("us", "env_evals_per_s", "bound", "frac")}
-            try:
-                secg = time_op_graph(torch, m, op, sets_s, 4096)
-                rg = op_report(desc, pk, op, secg, 4096)
-                small[op]["cuda_graph"] = {k: rg[k] for k in ("us", "env_evals_per_s", "frac")}
-            except Exception as ex:                      # graph capture is a convenience of the bench, not of the path
-                small[op]["cuda_graph"] = {"error": str(ex)[:120]}
-        # the whole step at B = 4096 through bard_step (fused kernel, or the four operators forked over side streams)
-        def steps_4096(n):
-            for i in range(n):
-                x = sets_s[i % len(sets_s)]
-                m.step(4096, x.q, x.qd, x.qdd, x.pose, x.J, x.tau, x.M, stream)
-        steps_4096(10)
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        barrier()
-        n0 = binding.launch_count()
-        e0.record()
-        steps_4096(200)
-        e1.record()
-        barrier()
-        us = e0.elapsed_time(e1) * 1e3 / 200
-        small["step"] = {"us": us, "env_evals_per_s": 4096 / (us * 1e-6), "launches_per_step": (binding.launch_count() - n0) / 200,
-                         "sum_of_operator_trains_us": sum(small[op]["us"] for op in OPS)}
-        del sets_s
+        try:
+            sec = time_graph(torch, m, op, sets, B)
+        except Exception:
+            sec = time_train(torch, m, op, sets, B, stream, launches=200)
+        ops[op]["train"] = short(op_report(desc, pk, op, sec, B), ("us", "frac", "achieved", "env_evals_per_s"))
     clocks.active.clear()
 
-    # ---- end to end: pinned host inputs -> device, four launches, every output -> pinned host, per step
+    # ---- end to end: pinned host inputs -> device, bard_step, every output -> pinned host, per step
     s0 = sets[0]
     h_in = [torch.empty(x.shape, dtype=x.dtype, pin_memory=True).copy_(x.cpu()) for x in (s0.q, s0.qd, s0.qdd)]
     d_out = (s0.pose, s0.J, s0.tau, s0.M)
@@ -457,25 +471,21 @@ def run_ours(args):
     for _ in range(Ke):
         e2e_step()
     barrier()
-    te = torch.tensor([time.perf_counter() - t0], device=dev, dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e = {"value": world * B * Ke / float(te.item()), "unit": UNIT, "h2d_bytes_per_step": h2d,
-           "d2h_bytes_per_step": d2h, "steps": Ke,
-           "note": "pinned host q/qd/qdd -> device, 4 launches, pose/J/tau/M -> pinned host, every step"}
-    clocks.stop()
+    te = D.max_over_ranks(time.perf_counter() - t0, dev)
+    e2e = {"value": world * B * Ke / te, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": Ke,
+           "note": "pinned host q/qd/qdd -> device, bard_step, pose/J/tau/M -> pinned host, every step (PCIe-bound)"}
+    del h_in, h_out
 
     dom = max(OPS, key=lambda o: op_sec[o])
-    d = ops[dom]
-    spec = (not args.no_specialize) and dom in SPEC_OPS
-    fused = launches == K
-    roof = {"kernel": f"bard_{dom}_n1 (model-specialised)" if spec else f"{dom}_kernel", "bound": d["bound"], "achieved": d["achieved"], "peak": d["peak"],
-            "unit": d["unit"], "frac": d["frac"], "traffic": None,
-            "peak_source": ("MEASURED_PEAKS.json hbm_gbs" if d["bound"] == "hbm" else
-                            "derived: 148 SM x 128 lanes x 2 x sm_max_mhz") + f" ({pk['source']})",
-            "algorithmic_per_launch": (d["bytes_per_env"] if d["bound"] == "hbm" else d["flop_per_env"]) * B,
-            "avg_launch_us": d["us"],
-            "timing": "CUDA events before every launch, second pass of K steps identical to the timed region"}
+    rd = op_report(desc, pk, dom, op_sec[dom], B)
+    spec = (not args.no_specialize)
+    roof = {"kernel": f"bard_{dom}_n1 (model-specialised)" if spec else f"{dom}_kernel", "bound": rd["bound"], "achieved": rd["achieved"],
+            "peak": rd["peak"], "unit": rd["unit"], "frac": rd["frac"], "traffic": None,
+            "peak_source": ("MEASURED_PEAKS.json hbm_gbs" if rd["bound"] == "hbm" else
+                            "min(measured FFMA chain, 148 SM x 128 lanes x 2 x sm_max_mhz)") + f" ({pk['source']})",
+            "algorithmic_per_launch": (rd["bytes_per_env"] if rd["bound"] == "hbm" else rd["flop_per_env"]) * B,
+            "avg_launch_us": rd["us"], "frac_back_to_back_train": ops[dom]["train"]["frac"],
+            "timing": "CUDA events before every launch, a second pass of K steps with the four operators called one by one"}
     tr = os.path.join(ROOT, "profiles", "traffic.json")   # dram bytes per launch from the committed ncu capture
     if os.path.exists(tr):
         try:
@@ -492,71 +502,166 @@ def run_ours(args):
                    "l2": f"{R} rotating buffer sets of {per_set / 1e6:.1f} MB (total {R * per_set / 1e6:.0f} MB > L2 126 MB)",
                    "layout": "SoA batch-fastest",
                    "specialized_ops": [] if args.no_specialize else list(SPEC_OPS),
-                   "step_call": "bard_step -> one fused kernel" if fused else "bard_step -> bard_fk, bard_jacobian, bard_rnea, bard_crba"},
-        "roofline": roof, "ops": ops, "ops_at_B4096": small, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks.summary(),
+                   "step_call": f"bard_step -> {launches / K:g} launch(es) per step"},
+        "roofline": roof, "ops": sig(ops), "e2e": e2e, "gpu_launches": int(launches),
+        "peaks": sig({"hbm_gbs": pk["hbm_gbs"], "fp32_tflops_used": pk["fp32_tflops"], "fp32_tflops_nominal": pk["fp32_tflops_nominal"],
+                      "fp32_tflops_measured_ffma_chain": pk["fp32_tflops_measured"], "source": pk["source"]}, 5),
     }
-    if args.sweep and rank == 0:
-        line["sweep"] = sweep(torch, binding, pk, dev, stream, specialize=not args.no_specialize)
-    if rank == 0 and world == 1 and not args.no_specialize and not args.no_rollout and m.nv > 0:
-        # SURVEY 8(f)2, beyond the four operators of the metric: ABA forward dynamics on the same workload (train timing)
-        try:
-            m.specialize(("aba",))
-            ws = torch.empty(m.aba_workspace_floats(B), device=dev)
-            qdd_out = torch.empty((m.nv, B), device=dev)
+    del sets
+    torch.cuda.empty_cache()
 
-            def aba_train(n):
-                for i in range(n):
-                    x = sets[i % R]
-                    m.aba(B, x.q, x.qd, x.tau, qdd_out, ws, stream)      # tau of the previous operators as the input torque
-            aba_train(5)
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            torch.cuda.synchronize()
-            e0.record()
-            aba_train(50)
-            e1.record()
-            torch.cuda.synchronize()
-            us = e0.elapsed_time(e1) * 1e3 / 50
-            io = 4 * (m.nq + 3 * m.nv)
-            line["aba"] = {"us": us, "env_evals_per_s": B / (us * 1e-6), "io_bytes_per_env": io, "workspace_bytes_per_env": 40 * m.nv,
-                           "hbm_gbs_io_plus_workspace": (io + 80 * m.nv) * B / (us * 1e-6) / 1e9,
-                           "note": "generated three-pass articulated-body kernel; not part of the headline metric"}
-            del ws, qdd_out
-        except Exception as ex:
-            line["aba"] = {"error": str(ex)[:200]}
-    if rank == 0 and world == 1 and not args.no_rollout:
-        try:
-            line["config2_rollout"] = rollout_config2(torch, binding, dev, specialize=not args.no_specialize)
-        except Exception as ex:                          # graph capture is a convenience of the bench, not of the path
-            line["config2_rollout"] = {"error": str(ex)[:200]}
+    if extras:
+        clocks.active.set()
+        # ---- BASELINE.json's metric: every operator and the step on configs 0-3 at B = 4096 and 65 536
+        if not args.no_matrix:
+            matrix = {}
+            for c in range(4):
+                dc, mc = model(c)
+                row = {}
+                for Bm in (4096, 65536):
+                    ss, _ = make_sets(torch, mc, dc, c, Bm, dev, min_sets=4, cap_bytes=8 << 30)
+                    cell = {}
+                    for op in OPS:
+                        r = op_report(dc, pk, op, time_graph(torch, mc, op, ss, Bm), Bm)
+                        cell[op] = short(r, ("us", "env_evals_per_s", "bound", "frac"))
+                    n0 = binding.launch_count()
+                    op_call(mc, "step", ss[0], Bm, stream)
+                    per = binding.launch_count() - n0
+                    sec = time_graph(torch, mc, "step", ss, Bm, launches=max(len(ss), 32))
+                    roof_us = sum(RL.roofline(dc, pk)[op]["t_env"] for op in OPS) * Bm * 1e6
+                    cell["step"] = {"us": sec * 1e6, "env_evals_per_s": Bm / sec, "launches": int(per), "sum_of_rooflines_us": roof_us,
+                                    "frac_of_summed_rooflines": roof_us / (sec * 1e6)}
+                    row[f"B{Bm}"] = cell
+                    del ss
+                    torch.cuda.empty_cache()
+                matrix[W.CONFIG_NAMES[c]] = row
+            line["matrix"] = sig(matrix)
+        # ---- BASELINE.json config 4: batch sweep on the humanoid and the chain, with the oracle's time per B
+        if not args.no_sweep:
+            import oracle
+            oracle.set_threads(os.cpu_count() or 1)
+            sweep = {}
+            for c in (3, 0):
+                dc, mc = model(c)
+                o = oracle.Oracle(dc)
+                n_or = 2048
+                oq, oqd, oqdd = (a.astype(np.float64) for a in W.config_states(c, n_or))
+                oracle_pass_seconds(o, oq, oqd, oqdd)
+                row = {}
+                for Bs in SWEEP_B:
+                    ss, _ = make_sets(torch, mc, dc, c, Bs, dev, cap_bytes=40 << 30)
+                    cell = {}
+                    for op in OPS:
+                        cell[op] = short(op_report(dc, pk, op, time_graph(torch, mc, op, ss, Bs), Bs))
+                    n = min(Bs, n_or)
+                    t = min(oracle_pass_seconds(o, oq[:, :n].copy(), oqd[:, :n].copy(), oqdd[:, :n].copy()) for _ in range(2))
+                    cell["oracle"] = {"s_for_B_est": t * Bs / n, "env_evals_per_s": n / t, "sample_envs": n}
+                    row[f"B{Bs}"] = cell
+                    del ss
+                    torch.cuda.empty_cache()
+                sweep[W.CONFIG_NAMES[c]] = row
+            sweep["note"] = (f"per operator: device time of a back-to-back train replayed from a CUDA graph, rotating buffer sets; oracle: fp64, "
+                             f"{oracle.get_threads()} host threads, all four operators on min(B, 2048) environments, scaled to B")
+            line["sweep"] = sig(sweep)
+        # ---- beyond the metric: ABA, RNEA VJP, fp64 / AoS variants, on the headline workload
+        if not args.no_specialize and m.nv > 0:
+            line.update(extras_section(torch, binding, m, desc, cfg, B, dev, stream, pk, spec_s))
+        if not args.no_rollout:
+            try:
+                d2, m2 = model(2)
+                line["config2_rollout"] = sig(rollout_config2(torch, binding, m2, d2, dev))
+            except Exception as ex:                      # graph capture is a convenience of the bench, not of the path
+                line["config2_rollout"] = {"error": str(ex)[:200]}
+        clocks.active.clear()
+    clocks.stop()
+    line["clocks"] = clocks.summary()
+    line["specialize_s"] = sig(spec_s, 3)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        cb, _, _ = time_oracle(desc, cfg, args.cpu_seconds)
-        line["cpu_baseline"] = cb
+        line["cpu_baseline"] = time_oracle(desc, cfg, 4.0 if args.quick else args.cpu_seconds)
+    line["bench_wall_s"] = round(time.perf_counter() - t_start, 1)
     if rank == 0:
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
 
 
-def sweep(torch, binding, pk, dev, stream, specialize=True):
-    """config 4: every operator on the humanoid and the chain at B = 1024 ... 1 048 576 (train timing)."""
+def extras_section(torch, binding, m, desc, cfg, B, dev, stream, pk, spec_s):
     out = {}
-    for cfg in (3, 0):
-        desc = W.config_robot(cfg)
-        m = binding.Model(desc, device=dev.index or 0)
-        if specialize:
-            m.specialize(SPEC_OPS)
-        for B in (1024, 4096, 16384, 65536, 262144, 1048576):
-            sets, _ = make_sets(torch, m, desc, cfg, B, dev, cap_bytes=40 << 30)
-            row = {}
+    sets, _ = make_sets(torch, m, desc, cfg, B, dev)
+
+    def timed(fn, n=30, warm=3):
+        for i in range(warm):
+            fn(i)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for i in range(n):
+            fn(i)
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) * 1e-3 / n
+
+    try:    # ABA forward dynamics
+        t0 = time.perf_counter()
+        m.specialize(("aba",))
+        spec_s["aba:" + desc.name] = time.perf_counter() - t0
+        ws = torch.empty(m.aba_workspace_floats(B), device=dev)
+        qdd_out = torch.empty((m.nv, B), device=dev)
+        sec = timed(lambda i: m.aba(B, sets[i % len(sets)].q, sets[i % len(sets)].qd, sets[i % len(sets)].qdd, qdd_out, ws, stream))
+        r = op_report(desc, pk, "aba", sec, B)
+        out["aba"] = {"us": sec * 1e6, "env_evals_per_s": B / sec, "roofline": short(r, ("bound", "achieved", "peak", "unit", "frac")),
+                      "bytes_per_env": r["bytes_per_env"], "flop_per_env": r["flop_per_env"],
+                      "workspace_bytes_per_env": 4 * m.aba_workspace_floats(B) // B}
+        del ws, qdd_out
+    except Exception as ex:
+        out["aba"] = {"error": str(ex)[:200]}
+    try:    # reverse-mode RNEA w.r.t. the inertial parameters: 4 input arrays, one outward pass
+        ws = torch.empty(max(1, m.rnea_vjp_workspace_floats(B)), device=dev)
+        g = torch.empty((m.nb, 10), device=dev)
+        sec = timed(lambda i: m.rnea_vjp_params(B, sets[i % len(sets)].q, sets[i % len(sets)].qd, sets[i % len(sets)].qdd,
+                                                sets[i % len(sets)].tau, g, ws, stream))
+        io = 4 * (m.nq + 3 * m.nv)
+        out["rnea_vjp"] = {"us": sec * 1e6, "env_evals_per_s": B / sec, "hbm_gbs": io * B / sec / 1e9, "bytes_per_env": io,
+                           "frac_of_hbm": io * B / sec / 1e9 / pk["hbm_gbs"], "launches": 2}
+        del ws, g
+    except Exception as ex:
+        out["rnea_vjp"] = {"error": str(ex)[:200]}
+    del sets
+    torch.cuda.empty_cache()
+    # fp64 / AoS variants of the four operators, train timing, own buffers
+    var = {}
+    try:
+        ins32 = W.sample_states(desc, B, seed=2000 + cfg)
+        for dtype, layout in (("f32", "aos"), ("f64", "soa")):
+            t0 = time.perf_counter()
+            m.specialize_variant(OPS, dtype, layout)
+            spec_s[f"{dtype}_{layout}:" + desc.name] = time.perf_counter() - t0
+            td = torch.float64 if dtype == "f64" else torch.float32
+            es = 8 if dtype == "f64" else 4
+            tin = [torch.from_numpy(a).to(dev).to(td) for a in ins32]
+            shapes = ((m.nb, 12), (m.nframes, 6, m.nv), (m.nv,), (m.nv, m.nv))
+            if layout == "aos":
+                tin = [t.t().contiguous() for t in tin]
+                outs = [torch.empty((B,) + sh, device=dev, dtype=td) for sh in shapes]
+            else:
+                outs = [torch.empty(sh + (B,), device=dev, dtype=td) for sh in shapes]
+            ws = torch.empty(max(m.variant_workspace_bytes(op, dtype, layout, B) for op in OPS) // 4 + 4, device=dev)
+            calls = {"fk": lambda i: m.fk_v(dtype, layout, B, tin[0], outs[0], ws, stream),
+                     "jacobian": lambda i: m.jacobian_v(dtype, layout, B, tin[0], outs[1], ws, stream),
+                     "rnea": lambda i: m.rnea_v(dtype, layout, B, tin[0], tin[1], tin[2], outs[2], ws, stream),
+                     "crba": lambda i: m.crba_v(dtype, layout, B, tin[0], outs[3], ws, stream)}
+            cell = {}
             for op in OPS:
-                sec = time_op_train(torch, m, op, sets, B, stream, launches=100)
-                r = op_report(desc, pk, op, sec, B)
-                row[op] = {k: r[k] for k in ("us", "env_evals_per_s", "bound", "frac", "hbm_gbs", "fp32_tflops")}
-            out[f"{W.CONFIG_NAMES[cfg]}_B{B}"] = row
-            del sets
+                sec = timed(calls[op], n=20)
+                c = RL.counts(desc)[op]
+                cell[op] = {"us": sec * 1e6, "hbm_gbs": c["bytes"] * (es // 4) * B / sec / 1e9, "tflops": c["flop"] * B / sec / 1e12}
+            var[f"{dtype}_{layout}"] = cell
+            del tin, outs, ws
             torch.cuda.empty_cache()
-        m.close()
-    return out
+        out["variants"] = var
+    except Exception as ex:
+        out["variants"] = {"error": str(ex)[:200]}
+    return sig(out)
 
 
 if __name__ == "__main__":

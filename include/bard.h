@@ -116,7 +116,7 @@ bard_status bard_model_set_frames(bard_model* m, int32_t nframes, const int32_t*
  * option "x" once from the environment variable BARD_X (upper case), bard_model_set_option overrides it; no operator
  * call reads the environment.  Keys (int64 values, -1 = the documented automatic rule): teams, pack, pack2_min_b,
  * pdl (team kernels); spec_min_b, spec_block, spec_roles_max_b, spec_crba_roles_max_b, spec_crba_roles_min_b,
- * spec_fused_max_rows, spec_fused_small_b, spec_kin_min_b, step_fork_max_b (which kernel a call gets: take effect at
+ * spec_fused_max_rows, spec_fused_small_b, spec_kin_min_b, step_fork_max_b, step_mode (which kernel a call gets: take effect at
  * the next operator call); spec_prefetch, spec_sync, spec_l2pf, spec_roles, spec_zero_role, spec_maxreg, spec_step4,
  * spec_step4_max_rows, spec_pair (code generation: take effect at the next bard_model_specialize).
  * section 10.  Unknown key: BARD_ERR_INVALID_ARG.  Not thread-safe against concurrent operator calls on the model. */
@@ -161,13 +161,17 @@ bard_status bard_rnea(const bard_model* m, int64_t B, const float* q, const floa
 bard_status bard_crba(const bard_model* m, int64_t B, const float* q, float* M, bard_stream stream);
 
 /* One simulation step's worth of operators on one batch: poses, Jacobians, torques and mass matrix of the same
- * (q, qd, qdd) -- the paper's tiered cache and "full pipeline" restated on chip.  If the model
- * was specialised with BARD_OP_FUSED and the batch is in the specialised regime, ONE kernel evaluates the joint
- * transforms and FK once per body and shares them between the four operators; otherwise bard_fk, bard_jacobian,
- * bard_rnea and bard_crba are enqueued on `stream` -- for small batches (B <= 16384, where one operator's grid does
- * not fill the machine) forked over three internal side streams and joined back into `stream`, so the step costs
- * its longest operator, not the sum; the fork-join is ordered after everything already in `stream`, is complete
- * before anything enqueued later, and can be captured into a CUDA graph.  Outputs and layouts as for the four calls. */
+ * (q, qd, qdd) -- the paper's tiered cache and "full pipeline" restated on chip.  The form is chosen
+ * per call from the batch size (option step_mode forces one):
+ *   B <= step_fork_max_b (16384): one operator's grid does not fill the machine, so bard_fk, bard_jacobian, bard_rnea and
+ *     bard_crba are FORKED over three internal side streams and joined back into `stream`: the step costs its longest
+ *     operator, not the sum; the fork-join is ordered after everything already in `stream`, is complete before anything
+ *     enqueued later, and can be captured into a CUDA graph (one capture at a time per model);
+ *   above, if the model was specialised with BARD_OP_FUSED: ONE launch -- the fused kernel that evaluates the joint
+ *     transforms and FK once per body and shares them between the four operators (robots with a small parked state), or
+ *     the operators side by side in one grid;
+ *   otherwise the four operators in sequence on `stream`.
+ * Outputs and layouts as for the four calls. */
 bard_status bard_step(const bard_model* m, int64_t B, const float* q, const float* qd, const float* qdd,
                       float* pose, float* J, float* tau, float* M, bard_stream stream);
 
@@ -193,24 +197,26 @@ bard_status bard_aba(const bard_model* m, int64_t B, const float* q, const float
 /* Precision and layout variants of the four operators.
  *   dtype : BARD_F32 (default) or BARD_F64 -- the whole recursion in double, model constants as the builder's unrounded
  *           doubles: the instantiation that reproduces the paper's fp64 agreement table (Table 1)
- *           against the fp64 oracle (<= 1e-11 on the BASELINE robots).
+ *           against the fp64 oracle (<= 1e-11 on the BASELINE robots).  Needs bard_model_specialize_variant(model, ops,
+ *           BARD_F64, layout) first (NVRTC, as bard_model_specialize); BARD_ERR_UNSUPPORTED otherwise.
  *   layout: BARD_LAYOUT_SOA (default: [rows][B], batch fastest) or BARD_LAYOUT_AOS -- the paper's batch-first layout
  *           (PAPER.md:103): q (B, nq), qd / qdd / tau (B, nv), pose (B, nb, 12), J (B, nframes, 6, nv), M (B, nv, nv),
- *           contiguous, so PyTorch callers pass their (B, n) tensors without a transpose.
- * bard_model_specialize_variant generates and compiles the operators in `ops` (BARD_OP_FK | JACOBIAN | RNEA | CRBA) for
- * that (dtype, layout) with NVRTC, as bard_model_specialize does; the _v calls launch them at every batch size (one
- * launch, asynchronous; pointers are device pointers to float or double according to dtype).  (BARD_F32,
- * BARD_LAYOUT_SOA) is the plain operator call.  Without the variant kernel: BARD_ERR_UNSUPPORTED.
- * bard_model_set_frames / set_inertial_params drop the variants that depend on them, like the plain kernels. */
+ *           contiguous, so PyTorch callers pass their (B, n) tensors as they are.  Served by tiled transposes around
+ *           the SoA kernels (1 + number of input arrays extra launches) through `workspace`: a caller-owned device
+ *           buffer of bard_variant_workspace_bytes(model, op, dtype, layout, B) bytes (0 / NULL for SoA).  B <= 2 097 120.
+ * All launches are asynchronous on `stream`; pointers are device pointers to float or double according to dtype.
+ * (BARD_F32, BARD_LAYOUT_SOA) is the plain operator call.  bard_model_set_frames / set_inertial_params drop the fp64
+ * kernels that depend on them, like the plain ones. */
 enum { BARD_F32 = 0, BARD_F64 = 1 };
 enum { BARD_LAYOUT_SOA = 0, BARD_LAYOUT_AOS = 1 };
 bard_status bard_model_specialize_variant(bard_model* m, uint32_t ops, int dtype, int layout);
 bard_status bard_model_variant_source(const bard_model* m, uint32_t op, int dtype, int layout, char* host_dst, size_t cap, size_t* need);
-bard_status bard_fk_v      (const bard_model* m, int dtype, int layout, int64_t B, const void* q, void* pose, bard_stream stream);
-bard_status bard_jacobian_v(const bard_model* m, int dtype, int layout, int64_t B, const void* q, void* J, bard_stream stream);
+size_t      bard_variant_workspace_bytes(const bard_model* m, uint32_t op, int dtype, int layout, int64_t B);
+bard_status bard_fk_v      (const bard_model* m, int dtype, int layout, int64_t B, const void* q, void* pose, void* workspace, bard_stream stream);
+bard_status bard_jacobian_v(const bard_model* m, int dtype, int layout, int64_t B, const void* q, void* J, void* workspace, bard_stream stream);
 bard_status bard_rnea_v    (const bard_model* m, int dtype, int layout, int64_t B, const void* q, const void* qd, const void* qdd,
-                            void* tau, bard_stream stream);
-bard_status bard_crba_v    (const bard_model* m, int dtype, int layout, int64_t B, const void* q, void* M, bard_stream stream);
+                            void* tau, void* workspace, bard_stream stream);
+bard_status bard_crba_v    (const bard_model* m, int dtype, int layout, int64_t B, const void* q, void* M, void* workspace, bard_stream stream);
 
 /* Reverse-mode derivative of RNEA with respect to the inertial parameters (the paper's
  * differentiable "functional mode", and its use: link masses identified through RNEA).
@@ -230,6 +236,10 @@ bard_status bard_rnea_vjp_params(const bard_model* m, int64_t B, const float* q,
  * ABA kernels, which have theta folded in as literals: the team kernels serve until bard_model_specialize runs again). */
 bard_status bard_model_inertial_params(const bard_model* m, double* host_params);
 bard_status bard_model_set_inertial_params(bard_model* m, const double* host_params);
+
+/* Utility for the roofline report: the device's plain-FP32 FMA throughput in TFLOP/s, measured
+ * with an FFMA-chain kernel (synchronous: allocates, launches, waits).  No operator depends on it. */
+bard_status bard_measure_fp32_peak(int cuda_device, double* tflops);
 
 const char* bard_status_string(bard_status s);
 const char* bard_last_error(void);

@@ -29,7 +29,7 @@ TABLES = {"LEVEL_PTR": (0, np.int32), "LEVEL_BODY": (1, np.int32), "BODY_LEVEL":
 EXPORTS = ["bard_model_create", "bard_model_destroy", "bard_model_dims", "bard_model_get_table",
            "bard_model_set_frames", "bard_model_set_option", "bard_model_get_option", "bard_model_specialize", "bard_model_specialized_source", "bard_fk", "bard_jacobian", "bard_rnea", "bard_crba", "bard_step", "bard_euler_step", "bard_aba", "bard_aba_workspace_floats", "bard_rnea_vjp_params", "bard_rnea_vjp_workspace_floats",
            "bard_model_inertial_params", "bard_model_set_inertial_params", "bard_model_specialize_variant", "bard_model_variant_source",
-           "bard_fk_v", "bard_jacobian_v", "bard_rnea_v", "bard_crba_v",
+           "bard_variant_workspace_bytes", "bard_fk_v", "bard_jacobian_v", "bard_rnea_v", "bard_crba_v", "bard_measure_fp32_peak",
            "bard_status_string", "bard_last_error", "bard_launch_count"]
 
 
@@ -84,10 +84,13 @@ def lib():
         L.bard_model_set_inertial_params.argtypes = [vp, C.POINTER(C.c_double)]
         L.bard_model_specialize_variant.argtypes = [vp, C.c_uint32, C.c_int, C.c_int]
         L.bard_model_variant_source.argtypes = [vp, C.c_uint32, C.c_int, C.c_int, C.c_char_p, C.c_size_t, C.POINTER(C.c_size_t)]
-        L.bard_fk_v.argtypes = [vp, C.c_int, C.c_int, i64, fp, fp, vp]
-        L.bard_jacobian_v.argtypes = [vp, C.c_int, C.c_int, i64, fp, fp, vp]
-        L.bard_rnea_v.argtypes = [vp, C.c_int, C.c_int, i64, fp, fp, fp, fp, vp]
-        L.bard_crba_v.argtypes = [vp, C.c_int, C.c_int, i64, fp, fp, vp]
+        L.bard_variant_workspace_bytes.argtypes = [vp, C.c_uint32, C.c_int, C.c_int, i64]
+        L.bard_variant_workspace_bytes.restype = C.c_size_t
+        L.bard_fk_v.argtypes = [vp, C.c_int, C.c_int, i64, fp, fp, fp, vp]
+        L.bard_jacobian_v.argtypes = [vp, C.c_int, C.c_int, i64, fp, fp, fp, vp]
+        L.bard_rnea_v.argtypes = [vp, C.c_int, C.c_int, i64, fp, fp, fp, fp, fp, vp]
+        L.bard_crba_v.argtypes = [vp, C.c_int, C.c_int, i64, fp, fp, fp, vp]
+        L.bard_measure_fp32_peak.argtypes = [C.c_int, C.POINTER(C.c_double)]
         L.bard_status_string.argtypes = [C.c_int]
         L.bard_status_string.restype = C.c_char_p
         L.bard_last_error.restype = C.c_char_p
@@ -99,6 +102,13 @@ def lib():
 def _check(code: int):
     if code != BARD_OK:
         raise BardError(code, lib().bard_last_error().decode())
+
+
+def measure_fp32_peak(device: int = 0) -> float:
+    """Measured plain-FP32 FMA throughput of the device in TFLOP/s (``bard_measure_fp32_peak``)."""
+    v = C.c_double()
+    _check(lib().bard_measure_fp32_peak(int(device), C.byref(v)))
+    return float(v.value)
 
 
 def launch_count() -> int:
@@ -247,17 +257,21 @@ class Model:
         _check(lib().bard_model_variant_source(self._h, OPS[op], DTYPES[dtype], LAYOUTS[layout], buf, need.value, C.byref(need)))
         return buf.value.decode()
 
-    def fk_v(self, dtype, layout, B, q, pose, stream=0):
-        _check(lib().bard_fk_v(self._h, DTYPES[dtype], LAYOUTS[layout], int(B), _ptr(q), _ptr(pose), stream or None))
+    def variant_workspace_bytes(self, op, dtype, layout, B) -> int:
+        return int(lib().bard_variant_workspace_bytes(self._h, OPS[op], DTYPES[dtype], LAYOUTS[layout], int(B)))
 
-    def jacobian_v(self, dtype, layout, B, q, J, stream=0):
-        _check(lib().bard_jacobian_v(self._h, DTYPES[dtype], LAYOUTS[layout], int(B), _ptr(q), _ptr(J), stream or None))
+    def fk_v(self, dtype, layout, B, q, pose, workspace=None, stream=0):
+        _check(lib().bard_fk_v(self._h, DTYPES[dtype], LAYOUTS[layout], int(B), _ptr(q), _ptr(pose), _ptr(workspace), stream or None))
 
-    def rnea_v(self, dtype, layout, B, q, qd, qdd, tau, stream=0):
-        _check(lib().bard_rnea_v(self._h, DTYPES[dtype], LAYOUTS[layout], int(B), _ptr(q), _ptr(qd), _ptr(qdd), _ptr(tau), stream or None))
+    def jacobian_v(self, dtype, layout, B, q, J, workspace=None, stream=0):
+        _check(lib().bard_jacobian_v(self._h, DTYPES[dtype], LAYOUTS[layout], int(B), _ptr(q), _ptr(J), _ptr(workspace), stream or None))
 
-    def crba_v(self, dtype, layout, B, q, M, stream=0):
-        _check(lib().bard_crba_v(self._h, DTYPES[dtype], LAYOUTS[layout], int(B), _ptr(q), _ptr(M), stream or None))
+    def rnea_v(self, dtype, layout, B, q, qd, qdd, tau, workspace=None, stream=0):
+        _check(lib().bard_rnea_v(self._h, DTYPES[dtype], LAYOUTS[layout], int(B), _ptr(q), _ptr(qd), _ptr(qdd), _ptr(tau),
+                                 _ptr(workspace), stream or None))
+
+    def crba_v(self, dtype, layout, B, q, M, workspace=None, stream=0):
+        _check(lib().bard_crba_v(self._h, DTYPES[dtype], LAYOUTS[layout], int(B), _ptr(q), _ptr(M), _ptr(workspace), stream or None))
 
     def rnea_vjp_workspace_floats(self, B) -> int:
         return int(lib().bard_rnea_vjp_workspace_floats(self._h, int(B)))

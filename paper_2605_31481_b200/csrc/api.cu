@@ -238,20 +238,29 @@ bard_status bard_step(const bard_model* bm, int64_t B, const float* q, const flo
                       float* tau, float* M, bard_stream stream) {
   if (!bm) { set_error("bard_step: model is NULL"); return BARD_ERR_INVALID_ARG; }
   bard::DeviceGuard guard(bm->m.device);
-  // the fused kernel needs all four outputs to exist; otherwise (no DOF, no frames, not specialised, small batch)
-  // the step is the four operators in sequence on the same stream
-  if (bm->m.nv > 0 && bm->m.nframes > 0) {
+  // Which form the step takes (measured on the BASELINE robots under CUDA-graph replay):
+  //  * small batches (B <= step_fork_max_b = 16384): one operator's grid does not fill the machine (B = 4096: 128 tiles
+  //    on 148 SMs) and the four operators are independent given (q, qd, qdd), so they are FORKED over three side
+  //    streams and joined: the step costs its longest operator, each operator running its own best small-batch kernel
+  //    (a fused straight-line kernel is one long dependent instruction stream there: quadruped at 4096: 25.9 us
+  //    fused, 7.4 us for its longest operator);
+  //  * above: ONE launch where the model has a one-launch kernel that pays at this batch (fused / side by side /
+  //    kinematics-fused + RNEA), else the four operators in sequence on the caller's stream.
+  // step_mode forces a form (tests, experiments).
+  const int64_t mode = bm->m.opt.step_mode;
+  const int64_t fork_max_b = bm->m.opt.step_fork_max_b;
+  StepFork& f = const_cast<bard_model*>(bm)->fj;
+  const bool want_fork = mode == 1 || (mode < 0 && B <= fork_max_b);
+  if (bm->m.nv > 0 && bm->m.nframes > 0 && (mode == 2 || (mode < 0 && !want_fork))) {
+    // a one-launch kernel needs all four outputs to exist
     bard_status s = check_call("bard_step", bm, B, q, qd, qdd, tau);
     if (s == BARD_OK) s = check_call("bard_step", bm, B, pose, J, M, M);
     if (s != BARD_OK || B == 0) return s;
     if (bard::launch_specialized(bm->m, BARD_OP_STEP, B, q, qd, qdd, pose, J, tau, M, stream, s)) return s;
   }
-  // Small batches: one operator's grid does not fill the machine (B = 4096: 128 tiles on 148 SMs), and the four
-  // operators are independent given (q, qd, qdd) -- fork them over three side streams and join, so the step costs
-  // its longest operator instead of the sum.  Works under stream capture (the side streams join the capture).
-  const int64_t fork_max_b = bm->m.opt.step_fork_max_b;
-  StepFork& f = const_cast<bard_model*>(bm)->fj;
-  if (f.ok && B > 0 && B <= fork_max_b && bm->m.nv > 0) {
+  if (f.ok && B > 0 && want_fork && bm->m.nv > 0) {
+    // Works under stream capture (the side streams join the capture).  One fork-join is enqueued at a time: the events
+    // are re-recorded by every call (a wait captures the event's state at the time of the call, so that is safe).
     std::lock_guard<std::mutex> lock(f.mu);
     cudaStream_t user = (cudaStream_t)stream;
     bool ok = cudaEventRecord(f.fork, user) == cudaSuccess;
@@ -300,12 +309,16 @@ bard_status bard_aba(const bard_model* bm, int64_t B, const float* q, const floa
 
 bard_status bard_model_specialize_variant(bard_model* bm, uint32_t ops, int dtype, int layout) {
   if (!bm) { set_error("bard_model_specialize_variant: model is NULL"); return BARD_ERR_INVALID_ARG; }
-  return bard::specialize_variant(bm->m, ops, dtype, layout);
+  if (dtype < 0 || dtype > 1 || layout < 0 || layout > 1) { set_error("bard_model_specialize_variant: unknown dtype / layout"); return BARD_ERR_INVALID_ARG; }
+  if (ops & ~(uint32_t)BARD_OP_STEP) { set_error("bard_model_specialize_variant: only BARD_OP_FK / JACOBIAN / RNEA / CRBA have variants"); return BARD_ERR_INVALID_ARG; }
+  // the layout needs no code of its own (transposes around the SoA kernels); fp32 variants are the plain kernels
+  return dtype == BARD_F64 ? bard::specialize_f64(bm->m, ops) : bard::specialize(bm->m, ops);
 }
 
 bard_status bard_model_variant_source(const bard_model* bm, uint32_t op, int dtype, int layout, char* host_dst, size_t cap, size_t* need) {
   if (!bm) { set_error("bard_model_variant_source: model is NULL"); return BARD_ERR_INVALID_ARG; }
-  const std::string* src = bard::variant_source(bm->m, op, dtype, layout);
+  (void)layout;
+  const std::string* src = dtype == BARD_F64 ? bard::f64_source(bm->m, op) : bard::specialized_source(bm->m, op);
   if (!src) { set_error("bard_model_variant_source: operator variant not specialised"); return BARD_ERR_INVALID_ARG; }
   if (need) *need = src->size() + 1;
   if (cap < src->size() + 1 || !host_dst) { set_error("bard_model_variant_source: destination too small"); return BARD_ERR_INVALID_ARG; }
@@ -313,38 +326,74 @@ bard_status bard_model_variant_source(const bard_model* bm, uint32_t op, int dty
   return BARD_OK;
 }
 
+static int64_t out_rows(const bard::Model& m, uint32_t op) {
+  return op == BARD_OP_FK ? 12 * (int64_t)m.nb : op == BARD_OP_JACOBIAN ? 6 * (int64_t)m.nframes * m.nv : op == BARD_OP_RNEA ? m.nv : (int64_t)m.nv * m.nv;
+}
+
+size_t bard_variant_workspace_bytes(const bard_model* bm, uint32_t op, int dtype, int layout, int64_t B) {
+  if (!bm || B <= 0 || layout != BARD_LAYOUT_AOS) return 0;
+  const bard::Model& m = bm->m;
+  const int64_t in_rows = m.nq + (op == BARD_OP_RNEA ? 2 * (int64_t)m.nv : 0);
+  return (size_t)(in_rows + out_rows(m, op)) * (size_t)B * (dtype == BARD_F64 ? 8 : 4) + 64;
+}
+
 // the _v calls: dtype / layout variants of the four operators.  (F32, SoA) is the plain call.
 static bard_status variant_call(const char* fn, const bard_model* bm, uint32_t op, int dtype, int layout, int64_t B, const void* q,
-                                const void* qd, const void* qdd, void* pose, void* J, void* tau, void* Mo, bard_stream stream) {
+                                const void* qd, const void* qdd, void* out, void* workspace, bard_stream stream) {
   if (!bm) { set_error(std::string(fn) + ": model is NULL"); return BARD_ERR_INVALID_ARG; }
   if (dtype < 0 || dtype > 1 || layout < 0 || layout > 1) { set_error(std::string(fn) + ": unknown dtype / layout"); return BARD_ERR_INVALID_ARG; }
   const bard::Model& m = bm->m;
   const bool empty = (op != BARD_OP_FK && m.nv == 0) || (op == BARD_OP_JACOBIAN && m.nframes == 0);
-  void* out = op == BARD_OP_FK ? pose : op == BARD_OP_JACOBIAN ? J : op == BARD_OP_RNEA ? tau : Mo;
   const void* dummy = bm;
   bard_status s = check_call(fn, bm, B, (m.nq == 0 || empty) ? dummy : q, (op == BARD_OP_RNEA && !empty) ? qd : dummy,
-                             (op == BARD_OP_RNEA && !empty) ? qdd : dummy, empty ? dummy : out);
+                             (op == BARD_OP_RNEA && !empty) ? qdd : dummy, empty ? dummy : (const void*)out);
   if (s != BARD_OK || B == 0 || empty) return s;
   bard::DeviceGuard guard(m.device);
-  return bard::launch_variant(m, op, dtype, layout, B, q, qd, qdd, pose, J, tau, Mo, stream);
+  const int es = dtype == BARD_F64 ? 8 : 4;
+  const void *sq = q, *sqd = qd, *sqdd = qdd;
+  void* sout = out;
+  if (layout == BARD_LAYOUT_AOS) {
+    // (B, n) -> [n][B] into the workspace, the SoA operator, [rows][B] -> (B, rows) into the caller's output
+    if (!workspace) { set_error(std::string(fn) + ": the AoS layout needs a workspace of bard_variant_workspace_bytes()"); return BARD_ERR_INVALID_ARG; }
+    char* w = reinterpret_cast<char*>((reinterpret_cast<uintptr_t>(workspace) + 15) & ~(uintptr_t)15);
+    auto take = [&](int64_t rows) { void* p = w; w += (size_t)rows * (size_t)B * es; return p; };
+    if (m.nq > 0) { void* p = take(m.nq); s = bard::launch_transpose(q, p, B, m.nq, es, stream); sq = p; }
+    if (op == BARD_OP_RNEA) {
+      void* p = take(m.nv);
+      if (s == BARD_OK) s = bard::launch_transpose(qd, p, B, m.nv, es, stream);
+      sqd = p;
+      p = take(m.nv);
+      if (s == BARD_OK) s = bard::launch_transpose(qdd, p, B, m.nv, es, stream);
+      sqdd = p;
+    }
+    if (s != BARD_OK) return s;
+    sout = take(out_rows(m, op));
+  }
+  if (dtype == BARD_F64) {
+    s = bard::launch_f64(m, op, B, sq, sqd, sqdd, op == BARD_OP_FK ? sout : nullptr, op == BARD_OP_JACOBIAN ? sout : nullptr,
+                         op == BARD_OP_RNEA ? sout : nullptr, op == BARD_OP_CRBA ? sout : nullptr, stream);
+  } else {
+    s = op == BARD_OP_FK ? bard_fk(bm, B, (const float*)sq, (float*)sout, stream)
+        : op == BARD_OP_JACOBIAN ? bard_jacobian(bm, B, (const float*)sq, (float*)sout, stream)
+        : op == BARD_OP_RNEA ? bard_rnea(bm, B, (const float*)sq, (const float*)sqd, (const float*)sqdd, (float*)sout, stream)
+                             : bard_crba(bm, B, (const float*)sq, (float*)sout, stream);
+  }
+  if (s == BARD_OK && layout == BARD_LAYOUT_AOS) s = bard::launch_transpose(sout, out, out_rows(m, op), B, es, stream);
+  return s;
 }
 
-bard_status bard_fk_v(const bard_model* bm, int dtype, int layout, int64_t B, const void* q, void* pose, bard_stream stream) {
-  if (dtype == BARD_F32 && layout == BARD_LAYOUT_SOA) return bard_fk(bm, B, (const float*)q, (float*)pose, stream);
-  return variant_call("bard_fk_v", bm, BARD_OP_FK, dtype, layout, B, q, nullptr, nullptr, pose, nullptr, nullptr, nullptr, stream);
+bard_status bard_fk_v(const bard_model* bm, int dtype, int layout, int64_t B, const void* q, void* pose, void* workspace, bard_stream stream) {
+  return variant_call("bard_fk_v", bm, BARD_OP_FK, dtype, layout, B, q, nullptr, nullptr, pose, workspace, stream);
 }
-bard_status bard_jacobian_v(const bard_model* bm, int dtype, int layout, int64_t B, const void* q, void* J, bard_stream stream) {
-  if (dtype == BARD_F32 && layout == BARD_LAYOUT_SOA) return bard_jacobian(bm, B, (const float*)q, (float*)J, stream);
-  return variant_call("bard_jacobian_v", bm, BARD_OP_JACOBIAN, dtype, layout, B, q, nullptr, nullptr, nullptr, J, nullptr, nullptr, stream);
+bard_status bard_jacobian_v(const bard_model* bm, int dtype, int layout, int64_t B, const void* q, void* J, void* workspace, bard_stream stream) {
+  return variant_call("bard_jacobian_v", bm, BARD_OP_JACOBIAN, dtype, layout, B, q, nullptr, nullptr, J, workspace, stream);
 }
 bard_status bard_rnea_v(const bard_model* bm, int dtype, int layout, int64_t B, const void* q, const void* qd, const void* qdd, void* tau,
-                        bard_stream stream) {
-  if (dtype == BARD_F32 && layout == BARD_LAYOUT_SOA) return bard_rnea(bm, B, (const float*)q, (const float*)qd, (const float*)qdd, (float*)tau, stream);
-  return variant_call("bard_rnea_v", bm, BARD_OP_RNEA, dtype, layout, B, q, qd, qdd, nullptr, nullptr, tau, nullptr, stream);
+                        void* workspace, bard_stream stream) {
+  return variant_call("bard_rnea_v", bm, BARD_OP_RNEA, dtype, layout, B, q, qd, qdd, tau, workspace, stream);
 }
-bard_status bard_crba_v(const bard_model* bm, int dtype, int layout, int64_t B, const void* q, void* M, bard_stream stream) {
-  if (dtype == BARD_F32 && layout == BARD_LAYOUT_SOA) return bard_crba(bm, B, (const float*)q, (float*)M, stream);
-  return variant_call("bard_crba_v", bm, BARD_OP_CRBA, dtype, layout, B, q, nullptr, nullptr, nullptr, nullptr, nullptr, M, stream);
+bard_status bard_crba_v(const bard_model* bm, int dtype, int layout, int64_t B, const void* q, void* M, void* workspace, bard_stream stream) {
+  return variant_call("bard_crba_v", bm, BARD_OP_CRBA, dtype, layout, B, q, nullptr, nullptr, M, workspace, stream);
 }
 
 size_t bard_rnea_vjp_workspace_floats(const bard_model* bm, int64_t B) {

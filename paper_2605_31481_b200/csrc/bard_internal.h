@@ -117,6 +117,7 @@ struct Specialized;           // specialize.cu: model-specialised (NVRTC) kernel
   X(spec_fused_small_b, -1)    /* ... and above it only up to this batch */                                    \
   X(spec_kin_min_b, -1)        /* smallest batch at which bard_step uses the kinematics-fused kernel + RNEA */ \
   X(step_fork_max_b, 16384)    /* bard_step forks the four operators over side streams up to this batch */     \
+  X(step_mode, -1)             /* bard_step: -1 auto, 0 four launches in sequence, 1 forked, 2 one-launch kernel */ \
   /* read by bard_model_specialize (code generation) */                                                        \
   X(spec_prefetch, 2)          /* bodies of input-load lookahead */                                            \
   X(spec_sync, -1)             /* bodies between CTA barriers (0 = none) */                                    \
@@ -194,10 +195,13 @@ void free_specialized(Specialized* s);
 const std::string* specialized_source(const Model& M, uint32_t op);
 bool launch_specialized(const Model& M, uint32_t op, int64_t B, const float* q, const float* qd, const float* qdd, float* pose,
                         float* J, float* tau, float* Mo, void* stream, bard_status& st);
-bard_status specialize_variant(Model& M, uint32_t ops, int dtype, int layout);
-const std::string* variant_source(const Model& M, uint32_t op, int dtype, int layout);
-bard_status launch_variant(const Model& M, uint32_t op, int dtype, int layout, int64_t B, const void* q, const void* qd, const void* qdd,
-                           void* pose, void* J, void* tau, void* Mo, void* stream);
+bard_status specialize_f64(Model& M, uint32_t ops);
+const std::string* f64_source(const Model& M, uint32_t op);
+bard_status launch_f64(const Model& M, uint32_t op, int64_t B, const void* q, const void* qd, const void* qdd, void* pose, void* J,
+                       void* tau, void* Mo, void* stream);
+
+// layout.cu: [rows][cols] -> [cols][rows] at HBM speed (elem = 4 or 8 bytes), one launch
+bard_status launch_transpose(const void* src, void* dst, int64_t rows, int64_t cols, int elem, void* stream);
 void drop_specialized_jacobian(Model& M);
 void drop_specialized_dynamics(Model& M);      // kernels with the inertial parameters folded in as literals
 

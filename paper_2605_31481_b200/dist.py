@@ -8,8 +8,9 @@ from __future__ import annotations
 
 
 def shard_range(B: int, rank: int, world: int) -> tuple[int, int]:
-    """Contiguous [lo, hi) of the batch axis owned by ``rank``; sizes differ by at most one and are rounded
-    to multiples of 4 environments where possible (keeps every SoA row slice 16-byte aligned)."""
+    """Contiguous [lo, hi) of the batch axis owned by ``rank``: every shard but the last holds ceil(B / world) rounded
+    up to a multiple of 4 environments (keeps every SoA row slice 16-byte aligned); the last takes what is left, and
+    trailing ranks can be EMPTY when B is small (B = 10, world = 4: 4, 4, 2, 0) -- an empty shard is a legal B = 0 call."""
     if world <= 1:
         return 0, B
     q = -(-B // world)

@@ -29,9 +29,11 @@ HBM_FALLBACK_GBS = 6650.0      # B200_PROFILING.md fallback
 SM_MAX_MHZ_FALLBACK = 1965.0
 
 
-def measured_peaks(root: str | None = None) -> dict:
+def measured_peaks(root: str | None = None, fp32_measured: float | None = None) -> dict:
     """HBM GB/s from MEASURED_PEAKS.json (driver-written) or the profiling guide's fallback; the plain-FP32
-    peak is derived: 148 SMs x 128 FMA lanes x 2 FLOP x max SM clock."""
+    peak is derived: 148 SMs x 128 FMA lanes x 2 FLOP x max SM clock.  If the caller measured
+    the FFMA throughput on the box (``binding.measure_fp32_peak``: an FFMA-chain kernel) both figures are recorded and
+    the "alu" roofline divides by min(measured, nominal) -- what the FMA pipes of THIS box deliver."""
     root = root or os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
     p = os.path.join(root, "MEASURED_PEAKS.json")
     hbm, mhz, src = HBM_FALLBACK_GBS, SM_MAX_MHZ_FALLBACK, "fallback"
@@ -41,8 +43,10 @@ def measured_peaks(root: str | None = None) -> dict:
             hbm, mhz, src = float(d["hbm_gbs"]), float(d.get("sm_max_mhz", mhz)), "measured"
         except Exception:
             pass
-    fp32 = SM_COUNT * FP32_LANES_PER_SM * 2 * mhz * 1e6 / 1e12
-    return {"hbm_gbs": hbm, "fp32_tflops": fp32, "sm_max_mhz": mhz, "source": src}
+    nominal = SM_COUNT * FP32_LANES_PER_SM * 2 * mhz * 1e6 / 1e12
+    fp32 = min(nominal, fp32_measured) if fp32_measured else nominal
+    return {"hbm_gbs": hbm, "fp32_tflops": fp32, "fp32_tflops_nominal": nominal, "fp32_tflops_measured": fp32_measured,
+            "sm_max_mhz": mhz, "source": src}
 
 
 def _ancestors(parent, i):
@@ -100,6 +104,21 @@ def counts(desc) -> dict:
             elif jt[j] == FREE:
                 crba += 42 * nd_i
 
+    # ABA, three passes, compact algebra, per body: joint transform; v (48) and c = v x S qd (24);
+    # p^A = v x* I v (72); U = I^A S (66), D (5), u (6), I^a = I^A - U U^T / D (48), p^a = p^A + I^a c + U u / D (78);
+    # X^T I^a X as rotate (I, M symmetric 75 each, H general 90) + translate (96) = 336, X^T p^a (42), accumulate (27);
+    # pass 3: a' = X a_p + c (48), qdd = (u - U^T a') / D (13), a = a' + S qdd (6).  Root bodies skip the parent terms;
+    # a free root solves a 6x6 SPD system instead (LDL^T ~ 200).
+    aba = 0
+    for i in range(nb):
+        root = parent[i] < 0
+        if jt[i] == FREE:
+            aba += 36 + 72 + 200 + 30
+        else:
+            has_dof = jt[i] != FIXED
+            aba += xform(jt[i]) + (0 if root else 48 + 24) + 72 + (66 + 5 + 6 if has_dof else 0)
+            aba += (0 if root else (48 if has_dof else 0) + 78 + 336 + 42 + 27) + (48 + (13 + 6 if has_dof else 0))
+
     def row(i, o, f):
         return {"in": i, "out": o, "bytes": i + o, "flop": f}
 
@@ -108,6 +127,7 @@ def counts(desc) -> dict:
         "jacobian": row(4 * nq, 24 * nf * nv, jac),
         "rnea": row(4 * (nq + 2 * nv), 4 * nv, rnea),
         "crba": row(4 * nq, 4 * nv * nv, crba),
+        "aba": row(4 * (nq + 2 * nv), 4 * nv, aba),
     }
 
 

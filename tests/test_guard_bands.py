@@ -36,6 +36,8 @@ def test_no_write_outside_the_outputs(cfg, B, path):
     dev = torch.device("cuda:0")
     m = binding.Model(desc, device=0)
     m.set_option("spec_min_b", (1 << 30) if path == "team" else 0)
+    if path in ("fused", "side_by_side"):
+        m.set_option("step_mode", 2)                         # the one-launch forms at every batch size
     if path == "fused":
         m.set_option("spec_fused_max_rows", 100000)
     if path == "side_by_side":

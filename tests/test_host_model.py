@@ -17,7 +17,7 @@ INT_TABLES = ["LEVEL_PTR", "LEVEL_BODY", "BODY_LEVEL", "PARENT_SLOT", "Q_OFF", "
 
 def test_library_exports_every_declared_symbol():
     hdr = open(os.path.join(ROOT, "include", "bard.h")).read()
-    declared = set(re.findall(r"\b(bard_[a-z_]+)\s*\(", hdr))
+    declared = set(re.findall(r"\b(bard_[a-z0-9_]+)\s*\(", hdr))
     assert declared == set(binding.EXPORTS)
     L = binding.lib()
     for name in declared:

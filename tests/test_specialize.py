@@ -287,7 +287,7 @@ def test_fused_step_matches_oracle_and_the_four_calls(idx):
     """bard_step: one fused kernel where it is built (small parked state), else the four operators; both against
     the oracle, and the fused outputs against the four specialised kernels bit for bit (same generated arithmetic)."""
     desc = _robots()[idx]
-    s = Spec(desc, spec_min_b=0, spec_fused_max_rows=100000)      # build the fused kernel for every robot here
+    s = Spec(desc, spec_min_b=0, spec_fused_max_rows=100000, step_mode=2)   # build the fused kernel for every robot here, use it at every B
     s.m.specialize(("fused",))
     q, qd, qdd = W.sample_states(desc, 700, seed=40 + idx)
     four = s.run(q, qd, qdd)
@@ -311,7 +311,7 @@ def test_side_by_side_step_is_one_launch_and_bit_equal_to_the_four_kernels(cfg, 
     (blockIdx.y = operator): the same generated code, so the same bits as the four separate launches."""
     desc = W.config_robot(cfg)
     # never the fused kernel, at any batch size; build the side-by-side kernel for every robot here
-    s = Spec(desc, spec_min_b=0, spec_fused_max_rows=0, spec_fused_small_b=0, spec_step4_max_rows=100000, spec_kin_min_b=1 << 40)
+    s = Spec(desc, spec_min_b=0, spec_fused_max_rows=0, spec_fused_small_b=0, spec_step4_max_rows=100000, spec_kin_min_b=1 << 40, step_mode=2)
     s.m.specialize(("fused",))
     q, qd, qdd = W.config_states(cfg, B)
     four = s.run(q, qd, qdd)

@@ -2,8 +2,8 @@
 
 fp64: the generated kernels typed on double with the builder's unrounded constants -- held to <= 1e-11 against the fp64
 oracle on the BASELINE robots, the paper's own way of validating (Table 1: 1000 random configurations
-per robot, max |delta| between two fp64 implementations).  AoS: the paper's batch-first layout -- same
-generated expressions as the SoA specialised kernels, so equal to them to 1-2 ulp after a transpose."""
+per robot, max |delta| between two fp64 implementations).  AoS: the paper's batch-first layout, served by
+tiled transposes around the SoA kernels -- bit-equal to the SoA call after a transpose, for every kernel family."""
 import re
 
 import numpy as np
@@ -30,24 +30,24 @@ def _robots():
 
 # ------------------------------------------------------------------------------------------- CPU
 @pytest.mark.parametrize("idx", [0, 3, 5, 6])
-def test_variant_sources_compile_on_host_and_cover_every_row(idx):
+def test_fp64_sources_compile_on_host_and_cover_every_row(idx):
     desc = _robots()[idx]
     m = binding.Model(desc, device=-1)
-    for dtype, layout in VARIANTS:
-        m.specialize_variant(ALL, dtype, layout)
-        for op, arr, n in (("fk", "pose", 12 * m.nb), ("crba", "Mo", m.nv * m.nv), ("jacobian", "J", 6 * m.nframes * m.nv), ("rnea", "tau", m.nv)):
-            src = m.variant_source(op, dtype, layout)
-            assert ("typedef double real;" in src) == (dtype == "f64")
-            assert ("#define IX(r, n) (e * (n) + (r))" in src) == (layout == "aos")
-            rows = sorted(int(r) for r in re.findall(r"strow\(%s, IX\((\d+)u, ROWS_%s\)" % (arr, arr), src))
-            assert rows == list(range(n)), (op, dtype, layout)
-            if dtype == "f64":                                   # no float literal may survive in an fp64 kernel body
-                body = src[src.index("op_body_"):]
-                assert not re.search(r"\d\.\d+(e[-+]?\d+)?f\b", body.replace("T(0.0f)", "").replace("T(1.0f)", ""))
+    m.specialize_variant(ALL, "f64", "soa")
+    for op, arr, n in (("fk", "pose", 12 * m.nb), ("crba", "Mo", m.nv * m.nv), ("jacobian", "J", 6 * m.nframes * m.nv), ("rnea", "tau", m.nv)):
+        src = m.variant_source(op, "f64", "soa")
+        assert "typedef double real;" in src and "#define REAL_F64 1" in src
+        rows = sorted(int(r) for r in re.findall(r"strow\(%s, IX\((\d+)u, ROWS_%s\)" % (arr, arr), src))
+        assert rows == list(range(n)), op
+        body = src[src.index("op_body_"):]                       # no float literal may survive in an fp64 kernel body
+        assert not re.search(r"\d\.\d+(e[-+]?\d+)?f\b", body.replace("T(0.0f)", "").replace("T(1.0f)", ""))
     with pytest.raises(binding.BardError):
         m.specialize_variant(("aba",), "f64", "soa")             # only the four operators have variants
     with pytest.raises(binding.BardError):
         m.fk_v("f64", "soa", 4, 1, 1)                            # host-only model: operators refuse to run
+    assert m.variant_workspace_bytes("crba", "f64", "soa", 100) == 0
+    assert m.variant_workspace_bytes("crba", "f64", "aos", 100) >= 8 * 100 * (m.nq + m.nv * m.nv)
+    assert m.variant_workspace_bytes("rnea", "f32", "aos", 100) >= 4 * 100 * (m.nq + 3 * m.nv)
 
 
 def test_set_frames_and_set_inertial_params_drop_the_dependent_variants():
@@ -68,10 +68,12 @@ torch = pytest.importorskip("torch")
 
 
 class Var:
-    def __init__(self, desc, dtype, layout):
+    def __init__(self, desc, dtype, layout, specialise=False):
         assert torch.cuda.is_available(), "GPU tests need CUDA; there is no CPU fallback"
         self.m = binding.Model(desc, device=0)
-        self.m.specialize_variant(ALL, dtype, layout)
+        if dtype == "f64" or specialise:
+            self.m.set_option("spec_min_b", 0)
+            self.m.specialize_variant(ALL, dtype, layout)
         self.dtype, self.layout = dtype, layout
         self.td = torch.float64 if dtype == "f64" else torch.float32
         self.dev = torch.device("cuda:0")
@@ -89,13 +91,16 @@ class Var:
         shapes = ((m.nb, 12), (m.nframes, 6, m.nv), (m.nv,), (m.nv, m.nv))
         outs = [torch.full(((B,) + sh) if aos else (sh + (B,)), float("nan"), device=dev, dtype=td) for sh in shapes]
         s = torch.cuda.current_stream().cuda_stream
+        ws = torch.full((max(m.variant_workspace_bytes(op, self.dtype, self.layout, B) for op in ALL) // 8 + 1,), float("nan"),
+                        device=dev, dtype=torch.float64)
         n0 = binding.launch_count()
-        m.fk_v(self.dtype, self.layout, B, tq, outs[0], s)
-        m.jacobian_v(self.dtype, self.layout, B, tq, outs[1], s)
-        m.rnea_v(self.dtype, self.layout, B, tq, tqd, tqdd, outs[2], s)
-        m.crba_v(self.dtype, self.layout, B, tq, outs[3], s)
+        m.fk_v(self.dtype, self.layout, B, tq, outs[0], ws, s)
+        m.jacobian_v(self.dtype, self.layout, B, tq, outs[1], ws, s)
+        m.rnea_v(self.dtype, self.layout, B, tq, tqd, tqdd, outs[2], ws, s)
+        m.crba_v(self.dtype, self.layout, B, tq, outs[3], ws, s)
         torch.cuda.synchronize()
-        assert binding.launch_count() - n0 == 4 or m.nv == 0 or m.nframes == 0
+        # SoA: one launch per operator; AoS: + one transpose per input array and one for the output
+        assert binding.launch_count() - n0 == (4 + 6 + 4 if aos else 4) or m.nv == 0 or m.nframes == 0 or m.nq == 0
         res = []
         for t in outs:
             a = t.cpu().numpy()
@@ -145,16 +150,13 @@ def test_table1_style_fp64_agreement(cfg):
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("specialise", [False, True])
 @pytest.mark.parametrize("idx", range(8))
-def test_aos_fp32_matches_oracle_and_the_soa_kernels(idx):
+def test_aos_fp32_matches_oracle_and_is_bit_equal_to_soa(idx, specialise):
+    """The batch-first layout needs no kernels of its own: team kernels (no NVRTC) and specialised kernels alike."""
     desc = _robots()[idx]
-    v = Var(desc, "f32", "aos")
+    v = Var(desc, "f32", "aos", specialise=specialise)
     o = oracle.Oracle(desc)
-    soa = binding.Model(desc, device=0)
-    soa.set_option("spec_min_b", 0)
-    soa.set_option("spec_roles_max_b", 0)                         # the plain one-thread-per-environment kernels
-    soa.set_option("spec_crba_roles_max_b", 0)
-    soa.specialize(ALL)
     dev = torch.device("cuda:0")
     for B in (1, 45, 1000 + 7):
         q, qd, qdd = W.sample_states(desc, B, seed=640 + idx)
@@ -163,14 +165,13 @@ def test_aos_fp32_matches_oracle_and_the_soa_kernels(idx):
             assert np.isfinite(a).all()
             assert nerr(a, r) <= tol
         tq, tqd, tqdd = (torch.from_numpy(a).to(dev) for a in (q, qd, qdd))
-        ref = [torch.empty(sh + (B,), device=dev) for sh in ((soa.nb, 12), (soa.nframes, 6, soa.nv), (soa.nv,), (soa.nv, soa.nv))]
+        m = v.m
+        ref = [torch.empty(sh + (B,), device=dev) for sh in ((m.nb, 12), (m.nframes, 6, m.nv), (m.nv,), (m.nv, m.nv))]
         s = torch.cuda.current_stream().cuda_stream
-        soa.fk(B, tq, ref[0], s); soa.jacobian(B, tq, ref[1], s); soa.rnea(B, tq, tqd, tqdd, ref[2], s); soa.crba(B, tq, ref[3], s)
+        m.fk(B, tq, ref[0], s); m.jacobian(B, tq, ref[1], s); m.rnea(B, tq, tqd, tqdd, ref[2], s); m.crba(B, tq, ref[3], s)
         torch.cuda.synchronize()
         for a, r in zip(out, ref):
-            # the same generated expressions behind another address map: equal up to the compiler's choice of which
-            # separate multiply + add pairs it contracts (it depends on the basic blocks the store form leaves), 1-2 ulp
-            assert nerr(a, r.cpu().numpy().astype(np.float64)) <= 2e-6
+            assert np.array_equal(a, r.cpu().numpy())              # the same kernels behind two transposes
 
 
 @pytest.mark.gpu
@@ -179,7 +180,7 @@ def test_variants_at_bench_size_sampled(dtype, layout):
     """Humanoid at B = 65 536 through every variant: a strided sample against the oracle, every element finite."""
     desc = W.config_robot(3)
     B = 65536
-    v = Var(desc, dtype, layout)
+    v = Var(desc, dtype, layout, specialise=True)
     o = oracle.Oracle(desc)
     q, qd, qdd = W.sample_states(desc, B, seed=2003, dtype=np.float64 if dtype == "f64" else np.float32)
     out = v.run(q, qd, qdd)
@@ -197,3 +198,6 @@ def test_variant_call_without_its_kernel_is_refused():
     with pytest.raises(binding.BardError) as e:
         m.fk_v("f64", "soa", 4, t, t)
     assert e.value.code == 3
+    with pytest.raises(binding.BardError) as e:
+        m.fk_v("f32", "aos", 4, t, t)                            # AoS without a workspace
+    assert e.value.code == 1
