@@ -65,6 +65,9 @@ def parse():
     ap.add_argument("--no-specialize", action="store_true",
                     help="skip bard_model_specialize: every operator runs its table-driven team kernel")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU work for the oracle baseline")
+    ap.add_argument("--only", default=None, choices=list(OPS) + ["step", "aba", "vjp"],
+                    help="profiling aid: a short train of ONE operator on --config / --B (rotating buffer sets), then exit")
+    ap.add_argument("--option", action="append", default=[], metavar="KEY=VALUE", help="bard_model_set_option before specialising (repeatable)")
     return ap.parse_args()
 
 
@@ -338,6 +341,50 @@ def rollout_config2(torch, binding, m, desc, dev, steps=24, dt=0.005, replays=10
                         "launches_per_24_steps": int(per_loop), "finite": bool(torch.isfinite(outs[3]).all())}
     out["note"] = "CUDA graph of 24 x (bard_step + bard_euler_step), dt 0.005, seeded qdd per step, median of 10 replays"
     return out
+
+
+def run_only(args):
+    """`--only op`: what the ncu captures under profiles/ run -- `--steps` launches of one operator after `--warmup`."""
+    import torch
+    from paper_2605_31481_b200 import binding
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    desc = W.config_robot(args.config)
+    m = binding.Model(desc, device=0)
+    for kv in args.option:
+        k, v = kv.split("=")
+        m.set_option(k, int(v))
+    if not args.no_specialize:
+        m.specialize(SPEC_OPS + (("aba",) if args.only == "aba" else ()))
+    B = args.B
+    sets, _ = make_sets(torch, m, desc, args.config, B, dev)
+    stream = torch.cuda.current_stream().cuda_stream
+    extra = {}
+    if args.only == "aba":
+        extra = {"ws": torch.empty(m.aba_workspace_floats(B), device=dev), "out": torch.empty((m.nv, B), device=dev)}
+    if args.only == "vjp":
+        extra = {"ws": torch.empty(max(1, m.rnea_vjp_workspace_floats(B)), device=dev), "out": torch.empty((m.nb, 10), device=dev)}
+
+    def call(i):
+        s = sets[i % len(sets)]
+        if args.only == "aba":
+            m.aba(B, s.q, s.qd, s.qdd, extra["out"], extra["ws"], stream)
+        elif args.only == "vjp":
+            m.rnea_vjp_params(B, s.q, s.qd, s.qdd, s.qdd, extra["out"], extra["ws"], stream)
+        else:
+            op_call(m, args.only, s, B, stream)
+
+    for i in range(max(3, args.warmup)):
+        call(i)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for i in range(args.steps):
+        call(i)
+    e1.record()
+    torch.cuda.synchronize()
+    print(json.dumps({"only": args.only, "config": W.CONFIG_NAMES[args.config], "B": B, "launches": args.steps,
+                      "us_per_launch_host_train": e0.elapsed_time(e1) * 1e3 / args.steps}), flush=True)
 
 
 def run_ours(args):
@@ -668,5 +715,7 @@ if __name__ == "__main__":
     a = parse()
     if a.impl == "reference":
         run_reference(a)
+    elif a.only:
+        run_only(a)
     else:
         run_ours(a)

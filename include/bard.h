@@ -116,9 +116,9 @@ bard_status bard_model_set_frames(bard_model* m, int32_t nframes, const int32_t*
  * option "x" once from the environment variable BARD_X (upper case), bard_model_set_option overrides it; no operator
  * call reads the environment.  Keys (int64 values, -1 = the documented automatic rule): teams, pack, pack2_min_b,
  * pdl (team kernels); spec_min_b, spec_block, spec_roles_max_b, spec_crba_roles_max_b, spec_crba_roles_min_b,
- * spec_fused_max_rows, spec_fused_small_b, spec_kin_min_b, step_fork_max_b, step_mode (which kernel a call gets: take effect at
+ * spec_fused_max_rows, spec_fused_small_b, spec_kin_min_b, spec_pack_min_b, spec_pack_max_b, step_fork_max_b, step_kin_fork, step_mode (which kernel a call gets: take effect at
  * the next operator call); spec_prefetch, spec_sync, spec_l2pf, spec_roles, spec_zero_role, spec_maxreg, spec_step4,
- * spec_step4_max_rows, spec_pair (code generation: take effect at the next bard_model_specialize).
+ * spec_step4_max_rows, spec_pack, spec_classical, spec_kin (code generation: take effect at the next bard_model_specialize).
  * section 10.  Unknown key: BARD_ERR_INVALID_ARG.  Not thread-safe against concurrent operator calls on the model. */
 bard_status bard_model_set_option(bard_model* m, const char* key, int64_t value);
 bard_status bard_model_get_option(const bard_model* m, const char* key, int64_t* value);
@@ -129,7 +129,9 @@ enum { BARD_OP_FK = 1, BARD_OP_JACOBIAN = 2, BARD_OP_RNEA = 4, BARD_OP_CRBA = 8,
        BARD_OP_FUSED = 16,    /* the fused kernel behind bard_step                                  */
        BARD_OP_ABA = 32,      /* forward dynamics (bard_aba): exists only as a specialised kernel   */
        BARD_OP_RNEA_ROLES = 64,   /* bard_model_specialized_source only: the limb-role RNEA kernel  */
-       BARD_OP_CRBA_ROLES = 128 }; /* bard_model_specialized_source only: the limb-role CRBA kernel */
+       BARD_OP_CRBA_ROLES = 128,  /* bard_model_specialized_source only: the limb-role CRBA kernel */
+       BARD_OP_RNEA_PACK2 = 256,  /* bard_model_specialized_source only: the RNEA kernel with two environments per thread */
+       BARD_OP_KIN = 512 };       /* bard_model_specialized_source only: the kinematics-fused kernel (FK + Jacobian + CRBA) */
 
 /* Model-specialised kernels (optional, once per model, takes seconds): writes straight-line CUDA source of
  * the operators in `ops` (BARD_OP_FUSED: one kernel that evaluates all four, see bard_step) for THIS model -- constants as literals, the tree walked depth first so that the
@@ -163,13 +165,14 @@ bard_status bard_crba(const bard_model* m, int64_t B, const float* q, float* M, 
 /* One simulation step's worth of operators on one batch: poses, Jacobians, torques and mass matrix of the same
  * (q, qd, qdd) -- the paper's tiered cache and "full pipeline" restated on chip.  The form is chosen
  * per call from the batch size (option step_mode forces one):
- *   B <= step_fork_max_b (16384): one operator's grid does not fill the machine, so bard_fk, bard_jacobian, bard_rnea and
+ *   B <= step_fork_max_b (256 x SM count): one operator's grid does not fill the machine, so bard_fk, bard_jacobian, bard_rnea and
  *     bard_crba are FORKED over three internal side streams and joined back into `stream`: the step costs its longest
  *     operator, not the sum; the fork-join is ordered after everything already in `stream`, is complete before anything
  *     enqueued later, and can be captured into a CUDA graph (one capture at a time per model);
  *   above, if the model was specialised with BARD_OP_FUSED: ONE launch -- the fused kernel that evaluates the joint
- *     transforms and FK once per body and shares them between the four operators (robots with a small parked state), or
- *     the operators side by side in one grid;
+ *     transforms and FK once per body and shares them between the four operators (robots with a small parked state) --
+ *     or TWO: the kinematics-fused kernel (FK + Jacobian + CRBA in one walk: they share q, poses and screws) and
+ *     bard_rnea on an internal side stream (ALU-bound beside an HBM-bound kernel), joined back into `stream`;
  *   otherwise the four operators in sequence on `stream`.
  * Outputs and layouts as for the four calls. */
 bard_status bard_step(const bard_model* m, int64_t B, const float* q, const float* qd, const float* qdd,

@@ -239,16 +239,18 @@ bard_status bard_step(const bard_model* bm, int64_t B, const float* q, const flo
   if (!bm) { set_error("bard_step: model is NULL"); return BARD_ERR_INVALID_ARG; }
   bard::DeviceGuard guard(bm->m.device);
   // Which form the step takes (measured on the BASELINE robots under CUDA-graph replay):
-  //  * small batches (B <= step_fork_max_b = 16384): one operator's grid does not fill the machine (B = 4096: 128 tiles
-  //    on 148 SMs) and the four operators are independent given (q, qd, qdd), so they are FORKED over three side
-  //    streams and joined: the step costs its longest operator, each operator running its own best small-batch kernel
-  //    (a fused straight-line kernel is one long dependent instruction stream there: quadruped at 4096: 25.9 us
-  //    fused, 7.4 us for its longest operator);
-  //  * above: ONE launch where the model has a one-launch kernel that pays at this batch (fused / side by side /
-  //    kinematics-fused + RNEA), else the four operators in sequence on the caller's stream.
+  //  * small batches (B <= step_fork_max_b = 256 x SMs = 8 warps of environments per SM): one operator's grid does not
+  //    fill the machine (B = 4096: 128 tiles on 148 SMs) and the four operators are independent given (q, qd, qdd), so
+  //    they are FORKED over three side streams and joined: the step costs about its longest operator, each operator
+  //    running its own best small-batch kernel (a fused straight-line kernel is one long dependent instruction stream
+  //    there: quadruped at 4096: 25.9 us fused, 7.4 us for its longest operator; humanoid at 32 768: 50 us forked, 77 us
+  //    in sequence);
+  //  * above: ONE launch where the model has a one-launch kernel that pays at this batch (fused / side by side), or TWO
+  //    (kinematics-fused kernel + RNEA on a side stream: humanoid at 65 536: 94.8 us against 103.8 us as four launches),
+  //    else the four operators in sequence on the caller's stream.
   // step_mode forces a form (tests, experiments).
   const int64_t mode = bm->m.opt.step_mode;
-  const int64_t fork_max_b = bm->m.opt.step_fork_max_b;
+  const int64_t fork_max_b = bm->m.opt.step_fork_max_b >= 0 ? bm->m.opt.step_fork_max_b : 256 * (int64_t)bm->m.sm_count;
   StepFork& f = const_cast<bard_model*>(bm)->fj;
   const bool want_fork = mode == 1 || (mode < 0 && B <= fork_max_b);
   if (bm->m.nv > 0 && bm->m.nframes > 0 && (mode == 2 || (mode < 0 && !want_fork))) {
@@ -257,6 +259,40 @@ bard_status bard_step(const bard_model* bm, int64_t B, const float* q, const flo
     if (s == BARD_OK) s = check_call("bard_step", bm, B, pose, J, M, M);
     if (s != BARD_OK || B == 0) return s;
     if (bard::launch_specialized(bm->m, BARD_OP_STEP, B, q, qd, qdd, pose, J, tau, M, stream, s)) return s;
+    // no full fused kernel for this robot / batch: kinematics-fused kernel + RNEA.  RNEA goes to a side stream when the
+    // fork plumbing exists (it is ALU-bound, the kinematics kernel HBM-bound: they overlap), else after it on `stream`.
+    if ((mode < 0 || mode == 2) && bard::kin_available(bm->m, B)) {
+      const bool side = f.ok && bm->m.opt.step_kin_fork != 0;
+      cudaStream_t user = (cudaStream_t)stream;
+      std::unique_lock<std::mutex> lock(f.mu, std::defer_lock);
+      bool forked = false;
+      if (side) {
+        lock.lock();
+        forked = cudaEventRecord(f.fork, user) == cudaSuccess && cudaStreamWaitEvent(f.side[1], f.fork, 0) == cudaSuccess;
+        if (!forked) cudaGetLastError();
+      }
+      bard_status sr = BARD_OK;
+      if (forked) sr = bard_rnea(bm, B, q, qd, qdd, tau, f.side[1]);      // first: it is short and fills the machine's ALUs early
+      if (bard::launch_kin(bm->m, B, q, pose, J, M, stream, s)) {
+        if (!forked) sr = bard_rnea(bm, B, q, qd, qdd, tau, stream);
+        else if (cudaEventRecord(f.join[1], f.side[1]) != cudaSuccess || cudaStreamWaitEvent(user, f.join[1], 0) != cudaSuccess) {
+          set_error(std::string("bard_step: fork-join: ") + cudaGetErrorString(cudaGetLastError()));
+          return BARD_ERR_CUDA;
+        }
+        return s != BARD_OK ? s : sr;
+      }
+      if (forked) {                                             // no kinematics kernel after all: join and run the rest in sequence
+        if (cudaEventRecord(f.join[1], f.side[1]) != cudaSuccess || cudaStreamWaitEvent(user, f.join[1], 0) != cudaSuccess) {
+          set_error(std::string("bard_step: fork-join: ") + cudaGetErrorString(cudaGetLastError()));
+          return BARD_ERR_CUDA;
+        }
+        lock.unlock();
+        bard_status t = bard_fk(bm, B, q, pose, stream);
+        if (t == BARD_OK) t = bard_jacobian(bm, B, q, J, stream);
+        if (t == BARD_OK) t = bard_crba(bm, B, q, M, stream);
+        return t != BARD_OK ? t : sr;
+      }
+    }
   }
   if (f.ok && B > 0 && want_fork && bm->m.nv > 0) {
     // Works under stream capture (the side streams join the capture).  One fork-join is enqueued at a time: the events

@@ -116,7 +116,8 @@ struct Specialized;           // specialize.cu: model-specialised (NVRTC) kernel
   X(spec_fused_max_rows, 112)  /* the fused step kernel is used at every batch up to this many parked rows */  \
   X(spec_fused_small_b, -1)    /* ... and above it only up to this batch */                                    \
   X(spec_kin_min_b, -1)        /* smallest batch at which bard_step uses the kinematics-fused kernel + RNEA */ \
-  X(step_fork_max_b, 16384)    /* bard_step forks the four operators over side streams up to this batch */     \
+  X(step_fork_max_b, -1)       /* bard_step forks the four operators over side streams up to this batch (auto: 256 x SMs) */ \
+  X(step_kin_fork, 1)          /* bard_step = kinematics-fused kernel + RNEA: RNEA on a side stream (1) or after it (0) */ \
   X(step_mode, -1)             /* bard_step: -1 auto, 0 four launches in sequence, 1 forked, 2 one-launch kernel */ \
   /* read by bard_model_specialize (code generation) */                                                        \
   X(spec_prefetch, 2)          /* bodies of input-load lookahead */                                            \
@@ -127,7 +128,11 @@ struct Specialized;           // specialize.cu: model-specialised (NVRTC) kernel
   X(spec_maxreg, 0)            /* --maxrregcount of the NVRTC compile (0 = none) */                            \
   X(spec_step4, 1)             /* build the side-by-side step kernel */                                        \
   X(spec_step4_max_rows, 72)                                                                                   \
-  X(spec_pair, -1)             /* RNEA: pack two components of one environment's 3-vectors per FFMA2 */
+  X(spec_kin, 1)               /* build the kinematics-fused kernel (FK + Jacobian + CRBA) with BARD_OP_FUSED */ \
+  X(spec_classical, 1)         /* RNEA of simple models in the classical Newton-Euler form about the COM (fewer FLOPs) */ \
+  X(spec_pack, 1)              /* RNEA: 2 = also build the kernel with two environments per thread (FFMA2); it loses: off */ \
+  X(spec_pack_min_b, -1)       /* ... and the batch range it is launched in */                                  \
+  X(spec_pack_max_b, -1)
 struct Options {
 #define BARD_OPT_FIELD(name, dflt) int64_t name = dflt;
   BARD_OPTIONS(BARD_OPT_FIELD)
@@ -202,6 +207,8 @@ bard_status launch_f64(const Model& M, uint32_t op, int64_t B, const void* q, co
 
 // layout.cu: [rows][cols] -> [cols][rows] at HBM speed (elem = 4 or 8 bytes), one launch
 bard_status launch_transpose(const void* src, void* dst, int64_t rows, int64_t cols, int elem, void* stream);
+bool kin_available(const Model& M, int64_t B);
+bool launch_kin(const Model& M, int64_t B, const float* q, float* pose, float* J, float* Mo, void* stream, bard_status& st);
 void drop_specialized_jacobian(Model& M);
 void drop_specialized_dynamics(Model& M);      // kernels with the inertial parameters folded in as literals
 

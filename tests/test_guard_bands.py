@@ -30,12 +30,15 @@ class Banded:
 
 
 @pytest.mark.parametrize("cfg,B", [(3, 1000 + 13), (1, 97), (0, 4096 + 1), (2, 33)])
-@pytest.mark.parametrize("path", ["team", "specialised", "fused", "side_by_side"])
+@pytest.mark.parametrize("path", ["team", "specialised", "fused", "side_by_side", "kin"])
 def test_no_write_outside_the_outputs(cfg, B, path):
     desc = W.config_robot(cfg)
     dev = torch.device("cuda:0")
     m = binding.Model(desc, device=0)
     m.set_option("spec_min_b", (1 << 30) if path == "team" else 0)
+    if path == "kin":                                        # kinematics-fused kernel + RNEA at every batch size
+        for k, v in (("spec_fused_max_rows", 0), ("spec_fused_small_b", 0), ("spec_step4", 0), ("spec_kin_min_b", 0), ("step_fork_max_b", 0)):
+            m.set_option(k, v)
     if path in ("fused", "side_by_side"):
         m.set_option("step_mode", 2)                         # the one-launch forms at every batch size
     if path == "fused":

@@ -327,6 +327,40 @@ def test_side_by_side_step_is_one_launch_and_bit_equal_to_the_four_kernels(cfg, 
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("cfg,B", [(3, 1000), (2, 777), (1, 300), (3, 65536)])
+@pytest.mark.parametrize("kin_fork", [1, 0])
+def test_kinematics_fused_step_matches_oracle_and_the_four_kernels(cfg, B, kin_fork):
+    """bard_step on the robots without a full fused kernel: FK + Jacobian + CRBA in ONE walk (they share q, poses and
+    screws) + bard_rnea (on a side stream or after it): two launches, every output against the oracle and against the four
+    separate specialised kernels (same generated expressions: equal to a few ulp)."""
+    desc = W.config_robot(cfg)
+    # never the full fused kernel / side-by-side grid; the kinematics kernel at every batch size
+    s = Spec(desc, spec_min_b=0, spec_fused_max_rows=0, spec_fused_small_b=0, spec_step4=0, spec_kin_min_b=0, step_fork_max_b=0,
+             step_kin_fork=kin_fork, spec_roles_max_b=0, spec_crba_roles_max_b=0)
+    s.m.specialize(("fused",))
+    assert "bard_kin_n1" in s.m.specialized_source("kin")
+    q, qd, qdd = W.config_states(cfg, B)
+    four = s.run(q, qd, qdd)
+    m, dev = s.m, s.dev
+    tq, tqd, tqdd = (torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in (q, qd, qdd))
+    outs = [torch.full(sh, float("nan"), device=dev) for sh in ((m.nb, 12, B), (m.nframes, 6, m.nv, B), (m.nv, B), (m.nv, m.nv, B))]
+    n0 = binding.launch_count()
+    m.step(B, tq, tqd, tqdd, *outs, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert binding.launch_count() - n0 == 2
+    got = [t.cpu().numpy() for t in outs]
+    idx = np.arange(0, B, max(1, B // 500))
+    ref = s.refs(*(a[:, idx] for a in (q, qd, qdd)))
+    for a, r, tol in zip(got, ref, (TOL_KIN, TOL_KIN, TOL_DYN, TOL_DYN)):
+        assert np.isfinite(a).all()
+        assert nerr(a[..., idx], r) <= tol
+    assert np.array_equal(got[3], np.swapaxes(got[3], 0, 1))
+    for a, b in zip(got, four):
+        assert nerr(a, b.astype(np.float64)) <= 1e-5
+    assert np.array_equal(got[2], four[2])                         # tau: the very same RNEA kernel
+
+
+@pytest.mark.gpu
 def test_step_without_specialisation_is_the_four_team_kernels():
     desc = W.config_robot(1)
     m = binding.Model(desc, device=0)
