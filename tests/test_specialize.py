@@ -1,6 +1,7 @@
 """Model-specialised kernels (bard_model_specialize): host-side generation + NVRTC compilation on CPU, and GPU
 parity of the generated FK / Jacobian / RNEA / CRBA against the fp64 oracle and against the level-parallel
 team kernels."""
+import os
 import re
 
 import numpy as np
@@ -11,6 +12,7 @@ from paper_2605_31481_b200 import binding, workloads as W
 
 TOL_KIN, TOL_DYN = 1e-4, 1e-3
 ALL = ("fk", "jacobian", "rnea", "crba")
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def nerr(x, ref):
@@ -543,3 +545,28 @@ def test_rnea_variant_without_l2_prefetch_matches(cfg):
         taus.append(tau.cpu().numpy())
         assert nerr(taus[-1], ref) <= TOL_DYN
     assert np.array_equal(taus[0], taus[1])
+
+
+def test_cubin_disk_cache_round_trip(tmp_path, monkeypatch):
+    """NVRTC output is cached on disk under $BARD_CACHE_DIR, keyed by hashes of (register cap, source): a second process
+    loads the file instead of compiling; a corrupt file is ignored (compiled again); BARD_CACHE=0 writes nothing."""
+    import subprocess
+    import sys
+    import time
+    code = ("import time, sys; sys.path.insert(0, %r)\n"
+            "from paper_2605_31481_b200 import binding, workloads as W\n"
+            "m = binding.Model(W.config_robot(1), device=-1)\n"
+            "t = time.perf_counter(); m.specialize(('crba',)); print(time.perf_counter() - t)\n") % ROOT
+    env = dict(__import__("os").environ, BARD_CACHE_DIR=str(tmp_path / "c"))
+    t1 = float(subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, check=True).stdout.split()[-1])
+    files = sorted((tmp_path / "c").glob("*.cubin"))
+    assert len(files) >= 1
+    t2 = float(subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, check=True).stdout.split()[-1])
+    assert t2 < 0.5 * t1                                           # no NVRTC run the second time
+    for f in files:
+        f.write_bytes(b"garbage")                                  # a damaged file: compile again, replace it
+    subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, check=True)
+    assert all(f.stat().st_size > 1000 for f in (tmp_path / "c").glob("*.cubin"))
+    env0 = dict(env, BARD_CACHE="0", BARD_CACHE_DIR=str(tmp_path / "off"))
+    subprocess.run([sys.executable, "-c", code], env=env0, capture_output=True, text=True, check=True)
+    assert not (tmp_path / "off").exists()
