@@ -390,6 +390,7 @@ def run_only(args):
 def run_ours(args):
     import torch
     import torch.distributed as dist
+    os.environ.setdefault("BARD_CACHE", "0")      # specialize_s reports NVRTC itself, not a warm on-disk cubin cache
     from paper_2605_31481_b200 import binding
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
