@@ -28,6 +28,7 @@ namespace bard {
 static thread_local std::string g_err;
 std::atomic<int64_t> g_launches{0};
 void set_error(const std::string& s) { g_err = s; }
+bool& launching_side_by_side() { static thread_local bool v = false; return v; }
 
 DeviceGuard::DeviceGuard(int device) {
   if (device < 0 || cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); return; }
@@ -272,8 +273,11 @@ bard_status bard_step(const bard_model* bm, int64_t B, const float* q, const flo
         if (!forked) cudaGetLastError();
       }
       bard_status sr = BARD_OK;
+      bard::launching_side_by_side() = forked;
       if (forked) sr = bard_rnea(bm, B, q, qd, qdd, tau, f.side[1]);      // first: it is short and fills the machine's ALUs early
-      if (bard::launch_kin(bm->m, B, q, pose, J, M, stream, s)) {
+      const bool kin_ok = bard::launch_kin(bm->m, B, q, pose, J, M, stream, s);
+      bard::launching_side_by_side() = false;
+      if (kin_ok) {
         if (!forked) sr = bard_rnea(bm, B, q, qd, qdd, tau, stream);
         else if (cudaEventRecord(f.join[1], f.side[1]) != cudaSuccess || cudaStreamWaitEvent(user, f.join[1], 0) != cudaSuccess) {
           set_error(std::string("bard_step: fork-join: ") + cudaGetErrorString(cudaGetLastError()));
@@ -302,10 +306,12 @@ bard_status bard_step(const bard_model* bm, int64_t B, const float* q, const flo
     bool ok = cudaEventRecord(f.fork, user) == cudaSuccess;
     for (int k = 0; k < 3 && ok; ++k) ok = cudaStreamWaitEvent(f.side[k], f.fork, 0) == cudaSuccess;
     if (ok) {
+      bard::launching_side_by_side() = true;                    // the four grids are meant to share the SMs
       bard_status s = bard_crba(bm, B, q, M, stream);           // the longest operator stays on the caller's stream
       bard_status s1 = bard_jacobian(bm, B, q, J, f.side[0]);
       bard_status s2 = bard_rnea(bm, B, q, qd, qdd, tau, f.side[1]);
       bard_status s3 = bard_fk(bm, B, q, pose, f.side[2]);
+      bard::launching_side_by_side() = false;
       for (int k = 0; k < 3; ++k)                               // always join, whatever the launches returned
         if (cudaEventRecord(f.join[k], f.side[k]) != cudaSuccess || cudaStreamWaitEvent(user, f.join[k], 0) != cudaSuccess) ok = false;
       if (!ok) { set_error(std::string("bard_step: fork-join: ") + cudaGetErrorString(cudaGetLastError())); return BARD_ERR_CUDA; }

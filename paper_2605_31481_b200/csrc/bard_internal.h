@@ -1,6 +1,7 @@
 // Internal definitions shared by the model builder (model.cu), the kernels (kernels.cu) and the C ABI
 // (api.cu).  Nothing here is used by oracle/.
 #pragma once
+#include <algorithm>
 #include <cstdint>
 #include <string>
 #include <vector>
@@ -128,6 +129,10 @@ struct Specialized;           // specialize.cu: model-specialised (NVRTC) kernel
   X(spec_maxreg, 0)            /* --maxrregcount of the NVRTC compile (0 = none) */                            \
   X(spec_step4, 1)             /* build the side-by-side step kernel */                                        \
   X(spec_step4_max_rows, 72)                                                                                   \
+  X(spec_ldnc, 1)              /* non-coherent (ld.global.nc) input loads in the generated kernels; 0 = coherent */ \
+  X(spec_pf_early, 1)          /* the up-front L2 prefetch burst in front of griddepcontrol.wait */ \
+  X(spec_max_block, 512)       /* __launch_bounds__ of the generated kernels (448: 144 registers instead of 128) */ \
+  X(spec_solo_smem, 1)         /* one-wave launches ask for > half of the shared memory: one CTA per SM also under PDL */ \
   X(spec_kin, 1)               /* build the kinematics-fused kernel (FK + Jacobian + CRBA) with BARD_OP_FUSED */ \
   X(spec_classical, 1)         /* RNEA of simple models in the classical Newton-Euler form about the COM (fewer FLOPs) */ \
   X(spec_pack, 1)              /* RNEA: 2 = also build the kernel with two environments per thread (FFMA2); it loses: off */ \
@@ -184,6 +189,16 @@ constexpr size_t kJBlobMax = sizeof(JHeader) + sizeof(FrameConst) * BARD_MAX_FRA
                              2 * (size_t)BARD_MAX_BODIES + 96;
 
 void set_error(const std::string& s);
+// Set (per host thread) by bard_step while it enqueues operators that are meant to run SIDE BY SIDE on several streams:
+// their launches must not ask for the shared memory that keeps an SM to one CTA (see solo_smem).
+bool& launching_side_by_side();
+// A launch whose grid fits one CTA per SM asks for more than half of the SM's shared memory, so that the plan (one CTA per
+// SM) also holds under programmatic dependent launch, where the next grid's CTAs are dispatched as resources free up:
+// where two CTAs fit an SM, the first SMs to finish take two of the next grid's CTAs and the last ones none (measured on
+// back-to-back trains: humanoid FK at B = 65 536 13 -> 23 us, quadruped Jacobian 18.8 -> 26.8 us, team CRBA at 4096 10.9 -> 15.2 us).
+inline size_t solo_smem(const Model& m, unsigned grid, size_t smem) {
+  return (grid <= (unsigned)m.sm_count && m.opt.spec_solo_smem && !launching_side_by_side()) ? std::max<size_t>(smem, 116 * 1024) : smem;
+}
 
 // kernels.cu
 bard_status launch_fk(const Model& m, int64_t B, const float* q, float* pose, void* stream);

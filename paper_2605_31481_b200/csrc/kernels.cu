@@ -1038,6 +1038,7 @@ bard_status launch_fk(const Model& m, int64_t B, const float* q, float* pose, vo
   std::string why;
   const bool p2 = B % 2 == 0 && aligned(q, 8) && aligned(pose, 8);
   if (!pick_cfg(m.opt, m.team_warps, B, m.common_bytes, m.nq + 12 * m.nslots, p2, std::max(12 * m.nb, m.nq), cfg, why)) return refuse("bard_fk", why);
+  cfg.smem = solo_smem(m, cfg.grid, cfg.smem);
   auto go = [&](auto kernel, auto id) {
     bard_status s = prep<decltype(id)::value>(kernel, "bard_fk");
     if (s != BARD_OK) return s;
@@ -1055,6 +1056,7 @@ bard_status launch_jacobian(const Model& m, int64_t B, const float* q, float* J,
                 std::max(6 * m.nframes * m.nv, m.nq), cfg, why))
     return refuse("bard_jacobian", why);
   const int vec_ok = (B % 4 == 0) && aligned(J, 16);
+  cfg.smem = solo_smem(m, cfg.grid, cfg.smem);
   auto go = [&](auto kernel, auto id) {
     bard_status s = prep<decltype(id)::value>(kernel, "bard_jacobian");
     if (s != BARD_OK) return s;
@@ -1076,6 +1078,7 @@ bard_status launch_rnea(const Model& m, int64_t B, const float* q, const float* 
   std::memcpy(map.q, m.rowmap_q, sizeof(map.q));
   std::memcpy(map.qd, m.rowmap_qd, sizeof(map.qd));
   std::memcpy(map.qdd, m.rowmap_qdd, sizeof(map.qdd));
+  cfg.smem = solo_smem(m, cfg.grid, cfg.smem);
   auto go = [&](auto kernel, auto id) {
     bard_status s = prep<decltype(id)::value>(kernel, "bard_rnea");
     if (s != BARD_OK) return s;
@@ -1093,6 +1096,7 @@ bard_status launch_crba(const Model& m, int64_t B, const float* q, float* M, voi
                 std::max(m.nv * m.nv, m.nq), cfg, why))
     return refuse("bard_crba", why);
   const int vec_ok = (B % 4 == 0) && aligned(M, 16);
+  cfg.smem = solo_smem(m, cfg.grid, cfg.smem);
   auto go = [&](auto kernel, auto id) {
     bard_status s = prep<decltype(id)::value>(kernel, "bard_crba");
     if (s != BARD_OK) return s;

@@ -40,17 +40,17 @@ def test_generated_source_compiles_on_host(idx):
         assert "bard_step_n1" in m.specialized_source("fused")       # written even where it is not worth building
     # FK: 12 rows per body; CRBA / Jacobian: every output row stored exactly once (fill + structural zeros)
     for op, arr, n in (("fk", "pose", 12 * m.nb), ("crba", "Mo", m.nv * m.nv), ("jacobian", "J", 6 * m.nframes * m.nv)):
-        rows = sorted(int(r) for r in re.findall(r"strow\(%s, IX\((\d+)u, ROWS_%s\)" % (arr, arr), m.specialized_source(op)))
+        rows = sorted(int(r) for r in re.findall(r"STROW\(%s, (\d+)u," % arr, m.specialized_source(op)))
         assert rows == list(range(n)), op
     src = m.specialized_source("rnea")
     # one outward and one inward section per body, every tau row stored exactly once
     assert len(re.findall(r"// ---- body \d+ \(outward\)", src)) == m.nb
     assert len(re.findall(r"// ---- body \d+ \(inward\)", src)) == m.nb
-    rows = sorted(int(r) for r in re.findall(r"strow\(tau, IX\((\d+)u, ROWS_tau\)", src))
+    rows = sorted(int(r) for r in re.findall(r"STROW\(tau, (\d+)u,", src))
     assert rows == list(range(m.nv))
     # every input row is loaded exactly once
     for arr, n in (("q", m.nq), ("qd", m.nv), ("qdd", m.nv)):
-        got = sorted(int(r) for r in re.findall(r"ldrow<T>\(%s, IX\((\d+)u, ROWS_%s\)\)" % (arr, arr), src))
+        got = sorted(int(r) for r in re.findall(r"LDROW\(%s, (\d+)u\)" % arr, src))
         assert got == list(range(n)), arr
 
 
@@ -119,7 +119,7 @@ def test_rnea_source_has_a_variant_without_l2_prefetch():
         m.set_option("spec_l2pf", int(v))
         m.specialize(("rnea",))
         src = m.specialized_source("rnea")
-        assert "_np(" not in src and ("pf_l2(q" in src) == (v == "1")
+        assert "_np(" not in src and ("PFROW(q" in src) == (v == "1")
 
 
 # ------------------------------------------------------------------------------------------- GPU

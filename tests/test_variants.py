@@ -37,7 +37,7 @@ def test_fp64_sources_compile_on_host_and_cover_every_row(idx):
     for op, arr, n in (("fk", "pose", 12 * m.nb), ("crba", "Mo", m.nv * m.nv), ("jacobian", "J", 6 * m.nframes * m.nv), ("rnea", "tau", m.nv)):
         src = m.variant_source(op, "f64", "soa")
         assert "typedef double real;" in src and "#define REAL_F64 1" in src
-        rows = sorted(int(r) for r in re.findall(r"strow\(%s, IX\((\d+)u, ROWS_%s\)" % (arr, arr), src))
+        rows = sorted(int(r) for r in re.findall(r"STROW\(%s, (\d+)u," % arr, src))
         assert rows == list(range(n)), op
         body = src[src.index("op_body_"):]                       # no float literal may survive in an fp64 kernel body
         assert not re.search(r"\d\.\d+(e[-+]?\d+)?f\b", body.replace("T(0.0f)", "").replace("T(1.0f)", ""))
