@@ -189,10 +189,12 @@ bard_status bard_euler_step(const bard_model* m, int64_t B, float dt, float* q, 
 /* ABA forward dynamics, the paper's fifth operator: qdd = M(q)^-1 (tau - C(q, qd)) by the
  * articulated-body algorithm -- three passes, the 6x6 update I^A_parent += X^T I^a X of PAPER.md:103 on the way up.
  * tau[nv][B] in, qdd[nv][B] out (free joint: [linear; angular] blocks as everywhere), gravity as in bard_rnea.
- * Needs bard_model_specialize(model, BARD_OP_ABA) first (there is no table-driven ABA kernel: BARD_ERR_UNSUPPORTED
- * otherwise, also for a free joint that is not on a root body) and a caller-owned device workspace of
- * bard_aba_workspace_floats(model, B) floats (10 nv B: what the downward acceleration pass needs of every body).
- * One launch, asynchronous. */
+ * Two kernels: after bard_model_specialize(model, BARD_OP_ABA) the generated one (per-body state on chip; a free joint
+ * must sit on a root body: BARD_ERR_UNSUPPORTED at specialisation otherwise); without it the table-driven one (any model,
+ * a free joint anywhere, no NVRTC; per-body state in the workspace: ~12 KB of traffic per environment, 4-7x slower).  `workspace`: a caller-owned
+ * device buffer of bard_aba_workspace_floats(model, B) floats -- 10 nv B with the generated kernel, 48 nb B without: ask
+ * AFTER specialising.  Every body with a DOF needs a positive-definite articulated inertia (a massless subtree under a
+ * joint divides by zero).  One launch, asynchronous. */
 size_t      bard_aba_workspace_floats(const bard_model* m, int64_t B);
 bard_status bard_aba(const bard_model* m, int64_t B, const float* q, const float* qd, const float* tau, float* qdd,
                      float* workspace, bard_stream stream);

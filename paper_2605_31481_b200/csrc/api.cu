@@ -336,7 +336,8 @@ bard_status bard_euler_step(const bard_model* bm, int64_t B, float dt, float* q,
 }
 
 size_t bard_aba_workspace_floats(const bard_model* bm, int64_t B) {
-  return (bm && B > 0) ? (size_t)10 * (size_t)bm->m.nv * (size_t)B : 0;
+  if (!bm || B <= 0) return 0;
+  return bard::aba_is_specialized(bm->m) ? (size_t)10 * (size_t)bm->m.nv * (size_t)B : bard::aba_generic_workspace_floats(bm->m, B);
 }
 
 bard_status bard_aba(const bard_model* bm, int64_t B, const float* q, const float* qd, const float* tau, float* qdd, float* workspace,

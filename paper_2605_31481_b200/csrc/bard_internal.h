@@ -227,6 +227,11 @@ bool launch_kin(const Model& M, int64_t B, const float* q, float* pose, float* J
 void drop_specialized_jacobian(Model& M);
 void drop_specialized_dynamics(Model& M);      // kernels with the inertial parameters folded in as literals
 
+// aba_generic.cu: the table-driven ABA (no NVRTC; a free joint anywhere)
+size_t aba_generic_workspace_floats(const Model& M, int64_t B);
+bard_status launch_aba_generic(const Model& M, int64_t B, const float* q, const float* qd, const float* tau, float* qdd, float* ws, void* stream);
+bool aba_is_specialized(const Model& M);
+
 // vjp.cu
 size_t rnea_vjp_workspace_floats(const Model& M, int64_t B);
 bard_status launch_rnea_vjp(const Model& M, int64_t B, const float* q, const float* qd, const float* qdd, const float* dtau,

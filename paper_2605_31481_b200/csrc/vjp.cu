@@ -26,53 +26,18 @@
 #include <string>
 
 #include "bard_internal.h"
+#include "dfs.h"
 
 namespace bard {
 extern std::atomic<int64_t> g_launches;
 
 namespace {
 
-struct VjpTab {
-  uint8_t order[BARD_MAX_BODIES];     // depth-first preorder
-  int8_t load[BARD_MAX_BODIES];       // per position: -2 world, -1 registers (parent = previous position), >= 0 slot
-  int8_t save[BARD_MAX_BODIES];       // per position: slot to save (v, a, lambda) to, -1 none
-};
-
-struct V3f { float x, y, z; };
-__device__ __forceinline__ V3f operator+(V3f a, V3f b) { return {a.x + b.x, a.y + b.y, a.z + b.z}; }
-__device__ __forceinline__ V3f cross(V3f a, V3f b) { return {a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x}; }
-__device__ __forceinline__ float dot(V3f a, V3f b) { return fmaf(a.z, b.z, fmaf(a.y, b.y, a.x * b.x)); }
-__device__ __forceinline__ V3f scale(float s, V3f a) { return {s * a.x, s * a.y, s * a.z}; }
-__device__ __forceinline__ V3f mulT(const float* R, V3f v) {        // R^T v
-  return {fmaf(R[6], v.z, fmaf(R[3], v.y, R[0] * v.x)), fmaf(R[7], v.z, fmaf(R[4], v.y, R[1] * v.x)), fmaf(R[8], v.z, fmaf(R[5], v.y, R[2] * v.x))};
-}
-
-// same reduction and polynomials as kernels.cu / the generated kernels (reading 16)
-__device__ __forceinline__ void sincos_fast(float x, float& s, float& c) {
-  const float kb = fmaf(x, 0.636619772367581343f, 12582912.0f);
-  const float k = kb - 12582912.0f;
-  const int qd = __float_as_int(kb);
-  float r = fmaf(k, -1.57079637050628662109375f, x);
-  r = fmaf(k, 4.371138828673793e-8f, r);
-  r = fmaf(k, 1.7151245100058819e-15f, r);
-  const float r2 = r * r;
-  float ps = fmaf(r2, -1.9515295891e-4f, 8.3321608736e-3f);
-  ps = fmaf(ps, r2, -1.6666654611e-1f);
-  ps = fmaf(ps * r2, r, r);
-  float pc = fmaf(r2, 2.443315711809948e-5f, -1.388731625493765e-3f);
-  pc = fmaf(pc, r2, 4.166664568298827e-2f);
-  pc = fmaf(pc * r2, r2, fmaf(r2, -0.5f, 1.0f));
-  const float ss = (qd & 1) ? pc : ps;
-  const float cc = (qd & 1) ? ps : pc;
-  s = __int_as_float(__float_as_int(ss) ^ ((qd & 2) << 30));
-  c = __int_as_float(__float_as_int(cc) ^ (((qd + 1) & 2) << 30));
-}
-
 struct State { V3f vw, vv, aw, av, lw, lv; };    // velocity, acceleration, pushed cotangent: [angular; linear]
 
 extern __shared__ __align__(16) float vsm[];
 
-__global__ void __launch_bounds__(256) rnea_vjp_kernel(const unsigned char* __restrict__ blob, uint32_t cwords, int nb, VjpTab tab,
+__global__ void __launch_bounds__(128) rnea_vjp_kernel(const unsigned char* __restrict__ blob, uint32_t cwords, int nb, DfsTab tab,
                                                        int nslots, uint32_t B, const float* __restrict__ q, const float* __restrict__ qd,
                                                        const float* __restrict__ qdd, const float* __restrict__ dtau,
                                                        float* __restrict__ partials) {
@@ -94,9 +59,21 @@ __global__ void __launch_bounds__(256) rnea_vjp_kernel(const unsigned char* __re
     const bool valid = e0 < B;
     const uint32_t e = valid ? e0 : B - 1;
     State cur = {};
+    // the four input scalars of a one-DOF joint are loaded one body ahead of their use (the walk is one dependent chain)
+    float nq = 0.f, nqd = 0.f, nqdd = 0.f, ndt = 0.f;
+    auto fetch = [&](int pos) {
+      if (pos >= nb) return;
+      const BodyConst& n = BC[tab.order[pos]];
+      if (n.type == BARD_JOINT_REVOLUTE || n.type == BARD_JOINT_PRISMATIC) {
+        nq = __ldg(q + (n.q_off * B + e)); nqd = __ldg(qd + (n.v_off * B + e)); nqdd = __ldg(qdd + (n.v_off * B + e)); ndt = __ldg(dtau + (n.v_off * B + e));
+      }
+    };
+    fetch(0);
     for (int pos = 0; pos < nb; ++pos) {
       const int i = tab.order[pos];
       const BodyConst& c = BC[i];
+      const float cq = nq, cqd = nqd, cqdd = nqdd, cdt = ndt;
+      fetch(pos + 1);
       const int ld = tab.load[pos];
       State P;
       if (ld == -1) P = cur;
@@ -134,17 +111,16 @@ __global__ void __launch_bounds__(256) rnea_vjp_kernel(const unsigned char* __re
         float u = 0.f, w = 0.f;
         if (c.type == BARD_JOINT_REVOLUTE) {
           float s, co;
-          sincos_fast(q[c.q_off * B + e], s, co);
+          sincos_fast(cq, s, co);
           u = s; w = 1.f - co;
         } else if (c.type == BARD_JOINT_PRISMATIC) {
-          u = q[c.q_off * B + e];
+          u = cq;
         }
 #pragma unroll
         for (int k = 0; k < 9; ++k) R[k] = fmaf(w, c.Bm[k], fmaf(u, c.A[k], c.R0[k]));
         t = {fmaf(w, c.b[0], fmaf(u, c.a[0], c.t0[0])), fmaf(w, c.b[1], fmaf(u, c.a[1], c.t0[1])), fmaf(w, c.b[2], fmaf(u, c.a[2], c.t0[2]))};
         if (c.type != BARD_JOINT_FIXED) {
-          const uint32_t vo = c.v_off * B + e;
-          const float x = qd[vo], y = qdd[vo], z = dtau[vo];
+          const float x = cqd, y = cqdd, z = cdt;
           const V3f Sw = {c.Sw[0], c.Sw[1], c.Sw[2]}, Sl = {c.Sl[0], c.Sl[1], c.Sl[2]};
           jw = scale(x, Sw); jv = scale(x, Sl); bw = scale(y, Sw); bv = scale(y, Sl); dw = scale(z, Sw); dv = scale(z, Sl);
         }
@@ -204,44 +180,13 @@ __global__ void vjp_reduce_kernel(const float* __restrict__ partials, int nparts
 
 constexpr size_t kSmemCap = 227 * 1024;
 
-struct Plan { VjpTab tab; int nslots; };
-
-Plan plan(const Model& M) {
-  Plan P = {};
-  std::vector<std::vector<int>> ch(M.nb);
-  for (int i = 0; i < M.nb; ++i)
-    if (M.parent[i] >= 0) ch[M.parent[i]].push_back(i);
-  std::vector<int> slot_of(M.nb, -1);
-  int pos = 0, prev = -1, maxslot = 0;
-  // iterative preorder; `depth` = number of branching proper ancestors
-  struct Item { int body, depth; };
-  std::vector<Item> stack;
-  for (int r = M.nb - 1; r >= 0; --r)
-    if (M.parent[r] < 0) stack.push_back({r, 0});
-  while (!stack.empty()) {
-    const Item it = stack.back();
-    stack.pop_back();
-    const int i = it.body, p = M.parent[i];
-    P.tab.order[pos] = (uint8_t)i;
-    P.tab.load[pos] = (int8_t)(p < 0 ? -2 : (p == prev ? -1 : slot_of[p]));
-    const bool branching = ch[i].size() >= 2;
-    P.tab.save[pos] = -1;
-    if (branching) { slot_of[i] = it.depth; P.tab.save[pos] = (int8_t)it.depth; maxslot = std::max(maxslot, it.depth + 1); }
-    for (int k = (int)ch[i].size() - 1; k >= 0; --k) stack.push_back({ch[i][k], it.depth + (branching ? 1 : 0)});
-    prev = i;
-    ++pos;
-  }
-  P.nslots = maxslot;
-  return P;
-}
-
 int vjp_grid(const Model& M, int64_t B, int block) {
   const int64_t tiles = (B + block - 1) / block;
   return (int)std::min<int64_t>(tiles, (int64_t)M.sm_count * 4);
 }
 int vjp_block(const Model& M, int nslots) {
   const size_t cbytes = sizeof(BlobHeader) + sizeof(BodyConst) * (size_t)M.nb;
-  for (int block : {256, 128, 64, 32}) {
+  for (int block : {128, 64, 32}) {
     const size_t smem = cbytes + (size_t)(block / 32) * M.nb * 10 * 4 + (size_t)nslots * 18 * block * 4;
     if (smem * (block >= 128 ? 2 : 1) <= kSmemCap) return block;     // two CTAs per SM where possible
   }
@@ -252,7 +197,7 @@ int vjp_block(const Model& M, int nslots) {
 
 size_t rnea_vjp_workspace_floats(const Model& M, int64_t B) {
   if (B <= 0) return 0;
-  const Plan P = plan(M);
+  const DfsPlan P = dfs_plan(M);
   const int block = std::max(32, vjp_block(M, P.nslots));
   return (size_t)vjp_grid(M, B, block) * (size_t)M.nb * 10;
 }
@@ -260,7 +205,7 @@ size_t rnea_vjp_workspace_floats(const Model& M, int64_t B) {
 bard_status launch_rnea_vjp(const Model& M, int64_t B, const float* q, const float* qd, const float* qdd, const float* dtau,
                             float* dparams, float* ws, void* stream) {
   if ((int64_t)std::max(M.nq, M.nv) * B >= ((int64_t)1 << 32)) { set_error("bard_rnea_vjp_params: an input array has 2^32 elements or more"); return BARD_ERR_UNSUPPORTED; }
-  const Plan P = plan(M);
+  const DfsPlan P = dfs_plan(M);
   const int block = vjp_block(M, P.nslots);
   if (!block) { set_error("bard_rnea_vjp_params: per-environment state does not fit in shared memory"); return BARD_ERR_UNSUPPORTED; }
   const int grid = vjp_grid(M, B, block), np = M.nb * 10;

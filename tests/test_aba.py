@@ -82,13 +82,14 @@ def test_oracle_aba_round_trip_through_rnea(idx):
     assert np.abs(o.rnea(q, qd, qdd) - tau).max() <= 1e-8 * max(1.0, np.abs(qdd).max())
 
 
-def test_aba_needs_specialisation_and_compiles_on_host():
+def test_aba_specialisation_compiles_on_host():
     m = binding.Model(W.config_robot(1), device=-1)
+    assert m.aba_workspace_floats(1000) == 48 * m.nb * 1000       # the table-driven kernel's per-body rows
     m.specialize(("aba",))
     src = m.specialized_source("aba")
     assert "bard_aba_n1" in src and src.count("(accelerations)") == m.nb
-    assert m.aba_workspace_floats(1000) == 10 * m.nv * 1000
-    # a free joint below another body: refused
+    assert m.aba_workspace_floats(1000) == 48 * m.nb * 1000       # host-only: nothing was loaded, nothing changes
+    # a free joint below another body: the generated kernel is refused (the table-driven one handles it)
     bad = W.build_robot("free_child", [-1, 0], [W.REVOLUTE, W.FREE], seed=2)
     mb = binding.Model(bad, device=-1)
     with pytest.raises(binding.BardError) as e:
@@ -108,13 +109,35 @@ def _robots():
     return out
 
 
+def _free_below():
+    """Free joints below other bodies (and a second root): only the table-driven kernel takes these."""
+    out = []
+    for seed in range(3):
+        d = W.random_tree(860 + seed, nb=6 + 2 * seed, shape=["random", "chain", "unbalanced"][seed], free_root=(seed == 1))
+        jt = d.joint_type.copy()
+        jt[2 + seed] = W.FREE
+        d.joint_type = jt
+        d.T_pre = d.T_pre.copy()
+        if d.T_post is not None:
+            d.T_post = d.T_post.copy()
+            d.T_post[2 + seed] = [1, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, 0]
+        out.append(d)
+    return out
+
+
 @pytest.mark.gpu
-@pytest.mark.parametrize("idx", range(10))
+@pytest.mark.parametrize("kernel", ["generated", "table"])
+@pytest.mark.parametrize("idx", range(13))
 @pytest.mark.parametrize("B", [1, 130, 1000 + 7])
-def test_gpu_aba_matches_oracle(idx, B):
-    desc = _robots()[idx]
+def test_gpu_aba_matches_oracle(idx, B, kernel):
+    robots = _robots() + _free_below()
+    desc = robots[idx]
+    if idx >= 10 and kernel == "generated":
+        pytest.skip("a free joint below another body: table-driven kernel only")
     m = binding.Model(desc, device=0)
-    m.specialize(("aba",))
+    if kernel == "generated":
+        m.specialize(("aba",))
+    assert m.aba_workspace_floats(B) == (10 * m.nv * B if kernel == "generated" and m.nv else 48 * m.nb * B)
     o = oracle.Oracle(desc)
     dev = torch.device("cuda:0")
     q, qd, tau = W.sample_states(desc, B, seed=300 + idx)
@@ -135,20 +158,22 @@ def test_gpu_aba_matches_oracle(idx, B):
 
 
 @pytest.mark.gpu
-def test_gpu_aba_without_specialisation_is_refused():
+def test_gpu_aba_null_workspace_is_refused():
     m = binding.Model(W.config_robot(0), device=0)
     t = torch.zeros(7, 8, device="cuda:0")
     with pytest.raises(binding.BardError) as e:
-        m.aba(8, t, t, t, t, t)
-    assert e.value.code == 3
+        m.aba(8, t, t, t, t, None)
+    assert e.value.code == 1
 
 
 @pytest.mark.gpu
-def test_gpu_aba_full_size_sampled():
+@pytest.mark.parametrize("kernel", ["generated", "table"])
+def test_gpu_aba_full_size_sampled(kernel):
     desc = W.config_robot(3)
     B = 65536
     m = binding.Model(desc, device=0)
-    m.specialize(("aba",))
+    if kernel == "generated":
+        m.specialize(("aba",))
     o = oracle.Oracle(desc)
     dev = torch.device("cuda:0")
     q, qd, tau = W.config_states(3, B)
