@@ -130,7 +130,6 @@ struct Specialized;           // specialize.cu: model-specialised (NVRTC) kernel
   X(spec_step4, 1)             /* build the side-by-side step kernel */                                        \
   X(spec_step4_max_rows, 72)                                                                                   \
   X(spec_ldnc, 1)              /* non-coherent (ld.global.nc) input loads in the generated kernels; 0 = coherent */ \
-  X(spec_pf_early, 1)          /* the up-front L2 prefetch burst in front of griddepcontrol.wait */ \
   X(spec_max_block, 512)       /* __launch_bounds__ of the generated kernels (448: 144 registers instead of 128) */ \
   X(spec_solo_smem, 1)         /* one-wave launches ask for > half of the shared memory: one CTA per SM also under PDL */ \
   X(spec_kin, 1)               /* build the kinematics-fused kernel (FK + Jacobian + CRBA) with BARD_OP_FUSED */ \
