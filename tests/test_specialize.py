@@ -557,7 +557,7 @@ def test_cubin_disk_cache_round_trip(tmp_path, monkeypatch):
             "from paper_2605_31481_b200 import binding, workloads as W\n"
             "m = binding.Model(W.config_robot(1), device=-1)\n"
             "t = time.perf_counter(); m.specialize(('crba',)); print(time.perf_counter() - t)\n") % ROOT
-    env = dict(__import__("os").environ, BARD_CACHE_DIR=str(tmp_path / "c"))
+    env = dict(os.environ, BARD_CACHE="1", BARD_CACHE_DIR=str(tmp_path / "c"))
     t1 = float(subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, check=True).stdout.split()[-1])
     files = sorted((tmp_path / "c").glob("*.cubin"))
     assert len(files) >= 1
