@@ -296,50 +296,81 @@ def short(r, keys=("us", "env_evals_per_s", "bound", "frac", "hbm_gbs", "fp32_tf
 
 def rollout_config2(torch, binding, m, desc, dev, steps=24, dt=0.005, replays=10):
     """BASELINE.json config 2: the 11-DOF spined quadruped, all four operators per simulated RL step (bard_step)
-    over 24 consecutive steps, q advanced on the device by explicit Euler (bard_euler_step) from seeded random qdd.
-    The 24-step loop is captured once into a CUDA graph and replayed; reported as env-steps/s."""
+    over 24 consecutive steps, q advanced on the device by explicit Euler from seeded random qdd.  The 24-step loop is
+    captured once into a CUDA graph and replayed; reported as env-steps/s.  Two forms: `serial` = bard_step then the
+    in-place bard_euler_step on one stream (each step waits for the integrator and the integrator for the step);
+    `pipelined` = the out-of-place bard_euler_step_to on a second stream over three rotating state buffers: the next state
+    depends on (q, qd, qdd) only, so the integrator runs beside the operators of its own step and leaves the critical path."""
     out = {}
     for B in (4096, 65536):
         q, qd, _ = W.sample_states(desc, B, seed=2002)
         q0, qd0 = torch.from_numpy(q).to(dev), torch.from_numpy(qd).to(dev)
-        tq, tqd = q0.clone(), qd0.clone()
         gen = torch.Generator(device=dev)
         gen.manual_seed(2002)
         qdds = [torch.randn((desc.nv, B), device=dev, generator=gen) for _ in range(steps)]
         outs = [torch.empty(sh, device=dev) for sh in ((m.nb, 12, B), (m.nframes, 6, m.nv, B), (m.nv, B), (m.nv, m.nv, B))]
+        tq = [q0.clone() for _ in range(3)]
+        tqd = [qd0.clone() for _ in range(3)]
+        side, eul = torch.cuda.Stream(), torch.cuda.Stream()
 
-        def loop(stream):
+        def serial():
             for k in range(steps):
-                m.step(B, tq, tqd, qdds[k], *outs, stream)
-                m.euler_step(B, dt, tq, tqd, qdds[k], stream)
+                m.step(B, tq[0], tqd[0], qdds[k], *outs, side.cuda_stream)
+                m.euler_step(B, dt, tq[0], tqd[0], qdds[k], side.cuda_stream)
 
-        side = torch.cuda.Stream()
-        side.wait_stream(torch.cuda.current_stream())
-        with torch.cuda.stream(side):
-            loop(side.cuda_stream)                       # warm-up (also loads every kernel before capture)
-        torch.cuda.current_stream().wait_stream(side)
-        torch.cuda.synchronize()
-        n0 = binding.launch_count()
-        g = torch.cuda.CUDAGraph()
-        with torch.cuda.graph(g, stream=side):
-            loop(side.cuda_stream)
-        per_loop = binding.launch_count() - n0
-        tq.copy_(q0); tqd.copy_(qd0)
-        g.replay()
-        torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        ms = []
-        for _ in range(replays):
-            tq.copy_(q0); tqd.copy_(qd0)                 # every replay integrates the same 24 steps
-            e0.record()
-            g.replay()
-            e1.record()
+        def pipelined():
+            start = torch.cuda.Event()
+            start.record(side)
+            eul.wait_event(start)
+            step_done, euler_done = [], []
+            for k in range(steps):
+                s, n = k % 3, (k + 1) % 3
+                if k > 0:
+                    side.wait_event(euler_done[k - 1])           # (q_k, qd_k) is ready
+                m.step(B, tq[s], tqd[s], qdds[k], *outs, side.cuda_stream)
+                ev = torch.cuda.Event()
+                ev.record(side)
+                step_done.append(ev)
+                if k >= 2:
+                    eul.wait_event(step_done[k - 2])             # buffer n held the state of step k - 2: its operators are done
+                m.euler_step_to(B, dt, tq[s], tqd[s], qdds[k], tq[n], tqd[n], eul.cuda_stream)
+                ev = torch.cuda.Event()
+                ev.record(eul)
+                euler_done.append(ev)
+            side.wait_event(euler_done[-1])
+
+        res = {}
+        for name, loop in (("serial", serial), ("pipelined", pipelined)):
+            side.wait_stream(torch.cuda.current_stream())
+            eul.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(side):
+                loop()                                       # warm-up (also loads every kernel before capture)
             torch.cuda.synchronize()
-            ms.append(e0.elapsed_time(e1))
-        med = float(np.median(ms))
-        out[f"B{B}"] = {"env_steps_per_s": B * steps / (med * 1e-3), "us_per_step": med * 1e3 / steps,
-                        "launches_per_24_steps": int(per_loop), "finite": bool(torch.isfinite(outs[3]).all())}
-    out["note"] = "CUDA graph of 24 x (bard_step + bard_euler_step), dt 0.005, seeded qdd per step, median of 10 replays"
+            n0 = binding.launch_count()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=side):
+                loop()
+            per_loop = binding.launch_count() - n0
+            tq[0].copy_(q0); tqd[0].copy_(qd0)
+            g.replay()
+            torch.cuda.synchronize()
+            final = (tq[steps % 3] if name == "pipelined" else tq[0]).clone()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            ms = []
+            for _ in range(replays):
+                tq[0].copy_(q0); tqd[0].copy_(qd0)           # every replay integrates the same 24 steps
+                e0.record()
+                g.replay()
+                e1.record()
+                torch.cuda.synchronize()
+                ms.append(e0.elapsed_time(e1))
+            med = float(np.median(ms))
+            res[name] = {"env_steps_per_s": B * steps / (med * 1e-3), "us_per_step": med * 1e3 / steps, "launches_per_24_steps": int(per_loop),
+                         "finite": bool(torch.isfinite(outs[3]).all()), "_final": final}
+        same = bool(torch.equal(res["serial"].pop("_final"), res["pipelined"].pop("_final")))
+        out[f"B{B}"] = dict(res["serial"], pipelined=dict(res["pipelined"], same_final_state_as_serial=same))
+    out["note"] = ("CUDA graph of 24 x (bard_step + Euler step), dt 0.005, seeded qdd per step, median of 10 replays; pipelined = "
+                   "bard_euler_step_to on a second stream over three rotating state buffers")
     return out
 
 

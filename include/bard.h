@@ -185,6 +185,13 @@ bard_status bard_step(const bard_model* m, int64_t B, const float* q, const floa
  * p += dt R(quat) v, quat += dt/2 quat (x) (omega, 0), renormalised.  One kernel launch, asynchronous. */
 bard_status bard_euler_step(const bard_model* m, int64_t B, float dt, float* q, float* qd, const float* qdd,
                             bard_stream stream);
+/* The same step OUT OF PLACE: (q, qd, qdd) -> (q_out, qd_out) (q_out == q and qd_out == qd is the in-place step; partial
+ * overlap is not allowed).  With two or three state buffers a rollout can integrate step k on one stream WHILE the
+ * operators of step k still read (q, qd) on another -- the next state depends on (q, qd, qdd) only (BASELINE.json config
+ * 2: "q advanced by explicit Euler from random qdd"), so the integrator leaves the critical path (bench.py,
+ * `config2_rollout.pipelined`). */
+bard_status bard_euler_step_to(const bard_model* m, int64_t B, float dt, const float* q, const float* qd, const float* qdd,
+                               float* q_out, float* qd_out, bard_stream stream);
 
 /* ABA forward dynamics, the paper's fifth operator: qdd = M(q)^-1 (tau - C(q, qd)) by the
  * articulated-body algorithm -- three passes, the 6x6 update I^A_parent += X^T I^a X of PAPER.md:103 on the way up.

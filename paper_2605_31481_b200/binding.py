@@ -27,7 +27,7 @@ TABLES = {"LEVEL_PTR": (0, np.int32), "LEVEL_BODY": (1, np.int32), "BODY_LEVEL":
           "PARENT_SLOT": (3, np.int32), "Q_OFF": (4, np.int32), "V_OFF": (5, np.int32), "DOF_BODY": (6, np.int32),
           "ANC_MASK": (7, np.uint64), "RODRIGUES": (8, np.float32)}
 EXPORTS = ["bard_model_create", "bard_model_destroy", "bard_model_dims", "bard_model_get_table",
-           "bard_model_set_frames", "bard_model_set_option", "bard_model_get_option", "bard_model_specialize", "bard_model_specialized_source", "bard_fk", "bard_jacobian", "bard_rnea", "bard_crba", "bard_step", "bard_euler_step", "bard_aba", "bard_aba_workspace_floats", "bard_rnea_vjp_params", "bard_rnea_vjp_workspace_floats",
+           "bard_model_set_frames", "bard_model_set_option", "bard_model_get_option", "bard_model_specialize", "bard_model_specialized_source", "bard_fk", "bard_jacobian", "bard_rnea", "bard_crba", "bard_step", "bard_euler_step", "bard_euler_step_to", "bard_aba", "bard_aba_workspace_floats", "bard_rnea_vjp_params", "bard_rnea_vjp_workspace_floats",
            "bard_model_inertial_params", "bard_model_set_inertial_params", "bard_model_specialize_variant", "bard_model_variant_source",
            "bard_variant_workspace_bytes", "bard_fk_v", "bard_jacobian_v", "bard_rnea_v", "bard_crba_v", "bard_measure_fp32_peak",
            "bard_status_string", "bard_last_error", "bard_launch_count"]
@@ -74,6 +74,7 @@ def lib():
         L.bard_crba.argtypes = [vp, i64, fp, fp, vp]
         L.bard_step.argtypes = [vp, i64, fp, fp, fp, fp, fp, fp, fp, vp]
         L.bard_euler_step.argtypes = [vp, i64, C.c_float, fp, fp, fp, vp]
+        L.bard_euler_step_to.argtypes = [vp, i64, C.c_float, fp, fp, fp, fp, fp, vp]
         L.bard_aba.argtypes = [vp, i64, fp, fp, fp, fp, fp, vp]
         L.bard_aba_workspace_floats.argtypes = [vp, i64]
         L.bard_aba_workspace_floats.restype = C.c_size_t
@@ -235,6 +236,10 @@ class Model:
     def euler_step(self, B, dt, q, qd, qdd, stream=0):
         """qd += dt qdd ; q (+)= dt qd in place (``bard_euler_step``)."""
         _check(lib().bard_euler_step(self._h, int(B), float(dt), _ptr(q), _ptr(qd), _ptr(qdd), stream or None))
+
+    def euler_step_to(self, B, dt, q, qd, qdd, q_out, qd_out, stream=0):
+        """(q_out, qd_out) = Euler step of (q, qd, qdd), out of place (``bard_euler_step_to``)."""
+        _check(lib().bard_euler_step_to(self._h, int(B), float(dt), _ptr(q), _ptr(qd), _ptr(qdd), _ptr(q_out), _ptr(qd_out), stream or None))
 
     def aba_workspace_floats(self, B) -> int:
         return int(lib().bard_aba_workspace_floats(self._h, int(B)))

@@ -332,7 +332,18 @@ bard_status bard_euler_step(const bard_model* bm, int64_t B, float dt, float* q,
   bard_status s = check_call("bard_euler_step", bm, B, q, bm->m.nv ? (const void*)qd : q, bm->m.nv ? (const void*)qdd : q, q);
   if (s != BARD_OK || B == 0) return s;
   bard::DeviceGuard guard(bm->m.device);
-  return bard::launch_euler(bm->m, B, dt, q, qd, qdd, stream);
+  return bard::launch_euler(bm->m, B, dt, q, qd, qdd, q, qd, stream);
+}
+
+bard_status bard_euler_step_to(const bard_model* bm, int64_t B, float dt, const float* q, const float* qd, const float* qdd, float* q_out,
+                               float* qd_out, bard_stream stream) {
+  if (!bm) { set_error("bard_euler_step_to: model is NULL"); return BARD_ERR_INVALID_ARG; }
+  if (bm->m.nq == 0) return check_call("bard_euler_step_to", bm, B, bm, bm, bm, bm);
+  bard_status s = check_call("bard_euler_step_to", bm, B, q, bm->m.nv ? (const void*)qd : q, bm->m.nv ? (const void*)qdd : q, q_out);
+  if (s == BARD_OK && B > 0 && bm->m.nv && !qd_out) { set_error("bard_euler_step_to: NULL device pointer"); s = BARD_ERR_INVALID_ARG; }
+  if (s != BARD_OK || B == 0) return s;
+  bard::DeviceGuard guard(bm->m.device);
+  return bard::launch_euler(bm->m, B, dt, q, qd, qdd, q_out, qd_out, stream);
 }
 
 size_t bard_aba_workspace_floats(const bard_model* bm, int64_t B) {

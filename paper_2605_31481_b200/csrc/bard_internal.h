@@ -205,7 +205,8 @@ bard_status launch_jacobian(const Model& m, int64_t B, const float* q, float* J,
 bard_status launch_rnea(const Model& m, int64_t B, const float* q, const float* qd, const float* qdd, float* tau,
                         void* stream);
 bard_status launch_crba(const Model& m, int64_t B, const float* q, float* M, void* stream);
-bard_status launch_euler(const Model& m, int64_t B, float dt, float* q, float* qd, const float* qdd, void* stream);
+bard_status launch_euler(const Model& m, int64_t B, float dt, const float* q, const float* qd, const float* qdd, float* q_out, float* qd_out,
+                         void* stream);
 
 
 // specialize.cu

@@ -896,9 +896,10 @@ __global__ void __launch_bounds__(256) crba_kernel(const void* __restrict__ gcom
 // table (type, q_off, v_off of every body) read from the constant blob in global memory (warp-uniform, cached).
 // Free joint: p += dt R(quat) v ; quat += dt/2 quat (x) (omega, 0) ; renormalised.  HBM-bound: 2 nv + nq rows in,
 // nv + nq rows out, every access one full line per warp.
+// qi / qdi: state in; qo_ / qdo: state out (the same pointers for the in-place step; no __restrict__ on them)
 __global__ void __launch_bounds__(256) euler_kernel(const unsigned char* __restrict__ blob, int nb, uint32_t B, float dt,
-                                                    float* __restrict__ q, float* __restrict__ qd,
-                                                    const float* __restrict__ qdd) {
+                                                    const float* qi, const float* qdi, const float* __restrict__ qdd,
+                                                    float* qo_, float* qdo) {
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   const uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;
   asm volatile("griddepcontrol.wait;" ::: "memory");
@@ -908,14 +909,14 @@ __global__ void __launch_bounds__(256) euler_kernel(const unsigned char* __restr
     const int t = bc[i].type;
     const uint32_t qo = (uint32_t)bc[i].q_off * B + e, vo = (uint32_t)bc[i].v_off * B + e;
     if (t == BARD_JOINT_REVOLUTE || t == BARD_JOINT_PRISMATIC) {
-      const float v = fmaf(dt, qdd[vo], qd[vo]);
-      qd[vo] = v;
-      q[qo] = fmaf(dt, v, q[qo]);
+      const float v = fmaf(dt, qdd[vo], qdi[vo]);
+      qdo[vo] = v;
+      qo_[qo] = fmaf(dt, v, qi[qo]);
     } else if (t == BARD_JOINT_FREE) {
       float tw[6];
 #pragma unroll
-      for (int k = 0; k < 6; ++k) { tw[k] = fmaf(dt, qdd[vo + k * B], qd[vo + k * B]); qd[vo + k * B] = tw[k]; }
-      float x = q[qo + 3 * B], y = q[qo + 4 * B], z = q[qo + 5 * B], w = q[qo + 6 * B];
+      for (int k = 0; k < 6; ++k) { tw[k] = fmaf(dt, qdd[vo + k * B], qdi[vo + k * B]); qdo[vo + k * B] = tw[k]; }
+      float x = qi[qo + 3 * B], y = qi[qo + 4 * B], z = qi[qo + 5 * B], w = qi[qo + 6 * B];
       const float n = rsqrtf(fmaf(x, x, fmaf(y, y, fmaf(z, z, w * w))));
       x *= n; y *= n; z *= n; w *= n;
       const float R[9] = {1.f - 2.f * (y * y + z * z), 2.f * (x * y - z * w), 2.f * (x * z + y * w),
@@ -923,12 +924,12 @@ __global__ void __launch_bounds__(256) euler_kernel(const unsigned char* __restr
                           2.f * (x * z - y * w), 2.f * (y * z + x * w), 1.f - 2.f * (x * x + y * y)};
 #pragma unroll
       for (int r = 0; r < 3; ++r)
-        q[qo + r * B] = fmaf(dt, fmaf(R[3 * r + 2], tw[2], fmaf(R[3 * r + 1], tw[1], R[3 * r] * tw[0])), q[qo + r * B]);
+        qo_[qo + r * B] = fmaf(dt, fmaf(R[3 * r + 2], tw[2], fmaf(R[3 * r + 1], tw[1], R[3 * r] * tw[0])), qi[qo + r * B]);
       const float h = 0.5f * dt, ox = tw[3], oy = tw[4], oz = tw[5];
       const float ex = fmaf(h, fmaf(w, ox, fmaf(y, oz, -z * oy)), x), ey = fmaf(h, fmaf(w, oy, fmaf(z, ox, -x * oz)), y),
                   ez = fmaf(h, fmaf(w, oz, fmaf(x, oy, -y * ox)), z), ew = fmaf(h, -fmaf(x, ox, fmaf(y, oy, z * oz)), w);
       const float m = rsqrtf(fmaf(ex, ex, fmaf(ey, ey, fmaf(ez, ez, ew * ew))));
-      q[qo + 3 * B] = ex * m; q[qo + 4 * B] = ey * m; q[qo + 5 * B] = ez * m; q[qo + 6 * B] = ew * m;
+      qo_[qo + 3 * B] = ex * m; qo_[qo + 4 * B] = ey * m; qo_[qo + 5 * B] = ez * m; qo_[qo + 6 * B] = ew * m;
     }
   }
 }
@@ -1023,14 +1024,15 @@ void launch(K kernel, const LaunchCfg& cfg, void* stream, Args... args) {
 
 }  // namespace
 
-bard_status launch_euler(const Model& m, int64_t B, float dt, float* q, float* qd, const float* qdd, void* stream) {
+bard_status launch_euler(const Model& m, int64_t B, float dt, const float* q, const float* qd, const float* qdd, float* q_out, float* qd_out,
+                         void* stream) {
   if ((int64_t)std::max(m.nq, m.nv) * B >= ((int64_t)1 << 32)) return refuse("bard_euler_step", "an input array has 2^32 elements or more");
   LaunchCfg cfg = {};
   cfg.pdl = m.opt.pdl != 0;
   cfg.threads = 256;
   cfg.grid = (unsigned)((B + 255) / 256);
   cfg.smem = 0;
-  launch(euler_kernel, cfg, stream, (const unsigned char*)m.d_blob, (int)m.nb, (uint32_t)B, dt, q, qd, qdd);
+  launch(euler_kernel, cfg, stream, (const unsigned char*)m.d_blob, (int)m.nb, (uint32_t)B, dt, q, qd, qdd, q_out, qd_out);
   return finish("bard_euler_step");
 }
 bard_status launch_fk(const Model& m, int64_t B, const float* q, float* pose, void* stream) {

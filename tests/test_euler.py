@@ -125,3 +125,23 @@ def test_config2_rollout_on_the_device():
         # the quaternion sign is free (q and -q are the same pose): compare poses through FK, velocities directly
         assert nerr(tqd.cpu().numpy(), oqd) <= 1e-5 * (step + 1)
         assert nerr(o.fk(tq.cpu().numpy().astype(np.float64)), o.fk(oq)) <= 1e-5 * (step + 1)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("cfg", [0, 2, 3])
+def test_out_of_place_euler_step_equals_the_in_place_one(cfg):
+    """bard_euler_step_to: same bits as bard_euler_step, inputs untouched, outputs fully written."""
+    desc = W.config_robot(cfg)
+    m = binding.Model(desc, device=0)
+    dev = torch.device("cuda:0")
+    B = 1000 + 13
+    q, qd, qdd = W.config_states(cfg, B)
+    tq, tqd, tqdd = (torch.from_numpy(a).to(dev) for a in (q, qd, qdd))
+    q2, qd2 = torch.full_like(tq, float("nan")), torch.full_like(tqd, float("nan"))
+    s = torch.cuda.current_stream().cuda_stream
+    m.euler_step_to(B, 0.005, tq, tqd, tqdd, q2, qd2, s)
+    torch.cuda.synchronize()
+    assert torch.equal(tq.cpu(), torch.from_numpy(q)) and torch.equal(tqd.cpu(), torch.from_numpy(qd))
+    m.euler_step(B, 0.005, tq, tqd, tqdd, s)
+    torch.cuda.synchronize()
+    assert torch.equal(q2, tq) and torch.equal(qd2, tqd)
