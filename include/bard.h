@@ -162,6 +162,13 @@ bard_status bard_rnea(const bard_model* m, int64_t B, const float* q, const floa
 /* CRBA: composite-inertia backward sweep (the X^T M X update of PAPER.md:103) and mass-matrix fill. */
 bard_status bard_crba(const bard_model* m, int64_t B, const float* q, float* M, bard_stream stream);
 
+/* The three operators that depend on q alone -- poses, Jacobians and the mass matrix -- of one batch.  They share joint
+ * transforms, world poses and screws (the paper's tiered cache: one FK evaluation shared by the queries): if
+ * the model was specialised with BARD_OP_FUSED and B > 256 x SM count, ONE kernel walks the tree once and stores all three
+ * (the kernel bard_step launches beside bard_rnea on the larger robots); otherwise bard_fk, bard_jacobian and bard_crba in
+ * sequence on `stream`.  Outputs and layouts as for the three calls. */
+bard_status bard_kinematics(const bard_model* m, int64_t B, const float* q, float* pose, float* J, float* M, bard_stream stream);
+
 /* One simulation step's worth of operators on one batch: poses, Jacobians, torques and mass matrix of the same
  * (q, qd, qdd) -- the paper's tiered cache and "full pipeline" restated on chip.  The form is chosen
  * per call from the batch size (option step_mode forces one):

@@ -27,7 +27,7 @@ TABLES = {"LEVEL_PTR": (0, np.int32), "LEVEL_BODY": (1, np.int32), "BODY_LEVEL":
           "PARENT_SLOT": (3, np.int32), "Q_OFF": (4, np.int32), "V_OFF": (5, np.int32), "DOF_BODY": (6, np.int32),
           "ANC_MASK": (7, np.uint64), "RODRIGUES": (8, np.float32)}
 EXPORTS = ["bard_model_create", "bard_model_destroy", "bard_model_dims", "bard_model_get_table",
-           "bard_model_set_frames", "bard_model_set_option", "bard_model_get_option", "bard_model_specialize", "bard_model_specialized_source", "bard_fk", "bard_jacobian", "bard_rnea", "bard_crba", "bard_step", "bard_euler_step", "bard_euler_step_to", "bard_aba", "bard_aba_workspace_floats", "bard_rnea_vjp_params", "bard_rnea_vjp_workspace_floats",
+           "bard_model_set_frames", "bard_model_set_option", "bard_model_get_option", "bard_model_specialize", "bard_model_specialized_source", "bard_fk", "bard_jacobian", "bard_rnea", "bard_crba", "bard_kinematics", "bard_step", "bard_euler_step", "bard_euler_step_to", "bard_aba", "bard_aba_workspace_floats", "bard_rnea_vjp_params", "bard_rnea_vjp_workspace_floats",
            "bard_model_inertial_params", "bard_model_set_inertial_params", "bard_model_specialize_variant", "bard_model_variant_source",
            "bard_variant_workspace_bytes", "bard_fk_v", "bard_jacobian_v", "bard_rnea_v", "bard_crba_v", "bard_measure_fp32_peak",
            "bard_status_string", "bard_last_error", "bard_launch_count"]
@@ -72,6 +72,7 @@ def lib():
         L.bard_jacobian.argtypes = [vp, i64, fp, fp, vp]
         L.bard_rnea.argtypes = [vp, i64, fp, fp, fp, fp, vp]
         L.bard_crba.argtypes = [vp, i64, fp, fp, vp]
+        L.bard_kinematics.argtypes = [vp, i64, fp, fp, fp, fp, vp]
         L.bard_step.argtypes = [vp, i64, fp, fp, fp, fp, fp, fp, fp, vp]
         L.bard_euler_step.argtypes = [vp, i64, C.c_float, fp, fp, fp, vp]
         L.bard_euler_step_to.argtypes = [vp, i64, C.c_float, fp, fp, fp, fp, fp, vp]
@@ -227,6 +228,10 @@ class Model:
 
     def rnea(self, B, q, qd, qdd, tau, stream=0):
         _check(lib().bard_rnea(self._h, int(B), _ptr(q), _ptr(qd), _ptr(qdd), _ptr(tau), stream or None))
+
+    def kinematics(self, B, q, pose, J, M, stream=0):
+        """Poses, Jacobians and mass matrix of one batch: one kernel where the kinematics-fused kernel exists (``bard_kinematics``)."""
+        _check(lib().bard_kinematics(self._h, int(B), _ptr(q), _ptr(pose), _ptr(J), _ptr(M), stream or None))
 
     def step(self, B, q, qd, qdd, pose, J, tau, M, stream=0):
         """All four operators of one (q, qd, qdd) batch: one fused kernel if specialised with "fused"."""

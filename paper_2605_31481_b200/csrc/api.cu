@@ -235,6 +235,20 @@ bard_status bard_crba(const bard_model* bm, int64_t B, const float* q, float* M,
   return bard::launch_crba(bm->m, B, q, M, stream);
 }
 
+bard_status bard_kinematics(const bard_model* bm, int64_t B, const float* q, float* pose, float* J, float* M, bard_stream stream) {
+  if (!bm) { set_error("bard_kinematics: model is NULL"); return BARD_ERR_INVALID_ARG; }
+  bard::DeviceGuard guard(bm->m.device);
+  if (bm->m.nv > 0 && bm->m.nframes > 0) {
+    bard_status s = check_call("bard_kinematics", bm, B, bm->m.nq ? (const void*)q : (const void*)pose, pose, J, M);
+    if (s != BARD_OK || B == 0) return s;
+    if (bard::launch_kin(bm->m, B, q, pose, J, M, stream, s)) return s;     // one walk, one launch
+  }
+  bard_status s = bard_fk(bm, B, q, pose, stream);
+  if (s == BARD_OK) s = bard_jacobian(bm, B, q, J, stream);
+  if (s == BARD_OK) s = bard_crba(bm, B, q, M, stream);
+  return s;
+}
+
 bard_status bard_step(const bard_model* bm, int64_t B, const float* q, const float* qd, const float* qdd, float* pose, float* J,
                       float* tau, float* M, bard_stream stream) {
   if (!bm) { set_error("bard_step: model is NULL"); return BARD_ERR_INVALID_ARG; }

@@ -128,6 +128,8 @@ def counts(desc) -> dict:
         "rnea": row(4 * (nq + 2 * nv), 4 * nv, rnea),
         "crba": row(4 * nq, 4 * nv * nv, crba),
         "aba": row(4 * (nq + 2 * nv), 4 * nv, aba),
+        # bard_kinematics: q read once; FK is part of CRBA's walk, the Jacobian adds its axis and column work
+        "kin": row(4 * nq, 48 * nb + 24 * nf * nv + 4 * nv * nv, crba + jac - sum(xform(jt[i]) + (63 if parent[i] >= 0 else 0) for i in used)),
     }
 
 

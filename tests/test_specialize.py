@@ -363,6 +363,33 @@ def test_kinematics_fused_step_matches_oracle_and_the_four_kernels(cfg, B, kin_f
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("cfg,B,specialised", [(3, 65536, True), (3, 1000, True), (1, 300, False), (2, 40000, True)])
+def test_bard_kinematics_matches_oracle(cfg, B, specialised):
+    """bard_kinematics: pose, J and M of one batch -- one launch of the kinematics-fused kernel where it exists and the
+    batch is in its regime, bard_fk + bard_jacobian + bard_crba otherwise; either way the three operators' results."""
+    desc = W.config_robot(cfg)
+    m = binding.Model(desc, device=0)
+    if specialised:
+        m.specialize(ALL + ("fused",))
+    o = oracle.Oracle(desc)
+    dev = torch.device("cuda:0")
+    q, _, _ = W.config_states(cfg, B)
+    tq = torch.from_numpy(q).to(dev)
+    outs = [torch.full(sh, float("nan"), device=dev) for sh in ((m.nb, 12, B), (m.nframes, 6, m.nv, B), (m.nv, m.nv, B))]
+    n0 = binding.launch_count()
+    m.kinematics(B, tq, *outs, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    one = specialised and B > 256 * 148 and "bard_kin_n1" in m.specialized_source("kin") if specialised and cfg != 1 else False
+    assert binding.launch_count() - n0 == (1 if one else 3)
+    idx = np.unique(np.concatenate([np.arange(0, B, max(1, B // 400)), [B - 1]]))
+    q64 = np.ascontiguousarray(q[:, idx].astype(np.float64))
+    for t, r, tol in zip(outs, (o.fk(q64), o.jacobian(q64), o.crba(q64)), (TOL_KIN, TOL_KIN, TOL_DYN)):
+        a = t.cpu().numpy()
+        assert np.isfinite(a).all()
+        assert nerr(a[..., idx], r) <= tol
+
+
+@pytest.mark.gpu
 def test_step_without_specialisation_is_the_four_team_kernels():
     desc = W.config_robot(1)
     m = binding.Model(desc, device=0)
