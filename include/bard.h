@@ -249,6 +249,19 @@ bard_status bard_crba_v    (const bard_model* m, int dtype, int layout, int64_t 
 size_t      bard_rnea_vjp_workspace_floats(const bard_model* m, int64_t B);
 bard_status bard_rnea_vjp_params(const bard_model* m, int64_t B, const float* q, const float* qd, const float* qdd,
                                  const float* dtau, float* dparams, float* workspace, bard_stream stream);
+/* The same operation for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): same arguments without `workspace`, same kernels, same bits.  The scratch is a
+ * static device array inside the library of BARD_VJP_STATIC_SCRATCH_FLOATS floats (1 MiB, held by every GPU that loads
+ * the library until the process exits); a call with bard_rnea_vjp_workspace_floats(model, B) above that is refused with
+ * BARD_ERR_UNSUPPORTED and a message (on a 148-SM GPU: more than 44 bodies at more than ~37 000 environments) -- use
+ * bard_rnea_vjp_params then.  The call makes no cudaMalloc / cudaFree and calls no allocating library routine.
+ * EVERY call on a device shares that one array: calls ordered on one stream are safe (nothing in the array has to start at
+ * zero: each call overwrites every entry it later reads), calls that OVERLAP on the GPU (two streams without an ordering
+ * between them) race on it and may return wrong sums.  The first call on a device looks the array's device address up
+ * (cudaGetSymbolAddress, once per device): make that call outside stream capture. */
+#define BARD_VJP_STATIC_SCRATCH_FLOATS 262144
+bard_status bard_rnea_vjp_params_static(const bard_model* m, int64_t B, const float* q, const float* qd, const float* qdd,
+                                        const float* dtau, float* dparams, bard_stream stream);
 /* The model's theta (HOST, [nb*10] doubles) as bard_model_create derived it from (mass, com, inertia) -- and its
  * replacement, for optimisation loops over the inertial parameters (system identification): a build-time call like
  * bard_model_set_frames (SYNCHRONISES the device, rewrites the constant tables, drops the generated RNEA / CRBA / step /

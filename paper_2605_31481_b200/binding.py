@@ -20,6 +20,7 @@ from . import build as _build
 BARD_OK = 0
 STATUS = {0: "BARD_OK", 1: "BARD_ERR_INVALID_ARG", 2: "BARD_ERR_TOPOLOGY", 3: "BARD_ERR_UNSUPPORTED",
           4: "BARD_ERR_ALLOC", 5: "BARD_ERR_CUDA"}
+VJP_STATIC_SCRATCH_FLOATS = 262144      # BARD_VJP_STATIC_SCRATCH_FLOATS in include/bard.h
 OPS = {"fk": 1, "jacobian": 2, "rnea": 4, "crba": 8, "fused": 16, "aba": 32, "rnea_roles": 64, "crba_roles": 128, "rnea_pack2": 256, "kin": 512}
 DTYPES = {"f32": 0, "f64": 1}
 LAYOUTS = {"soa": 0, "aos": 1}
@@ -27,7 +28,7 @@ TABLES = {"LEVEL_PTR": (0, np.int32), "LEVEL_BODY": (1, np.int32), "BODY_LEVEL":
           "PARENT_SLOT": (3, np.int32), "Q_OFF": (4, np.int32), "V_OFF": (5, np.int32), "DOF_BODY": (6, np.int32),
           "ANC_MASK": (7, np.uint64), "RODRIGUES": (8, np.float32)}
 EXPORTS = ["bard_model_create", "bard_model_destroy", "bard_model_dims", "bard_model_get_table",
-           "bard_model_set_frames", "bard_model_set_option", "bard_model_get_option", "bard_model_specialize", "bard_model_specialized_source", "bard_fk", "bard_jacobian", "bard_rnea", "bard_crba", "bard_kinematics", "bard_step", "bard_euler_step", "bard_euler_step_to", "bard_aba", "bard_aba_workspace_floats", "bard_rnea_vjp_params", "bard_rnea_vjp_workspace_floats",
+           "bard_model_set_frames", "bard_model_set_option", "bard_model_get_option", "bard_model_specialize", "bard_model_specialized_source", "bard_fk", "bard_jacobian", "bard_rnea", "bard_crba", "bard_kinematics", "bard_step", "bard_euler_step", "bard_euler_step_to", "bard_aba", "bard_aba_workspace_floats", "bard_rnea_vjp_params", "bard_rnea_vjp_params_static", "bard_rnea_vjp_workspace_floats",
            "bard_model_inertial_params", "bard_model_set_inertial_params", "bard_model_specialize_variant", "bard_model_variant_source",
            "bard_variant_workspace_bytes", "bard_fk_v", "bard_jacobian_v", "bard_rnea_v", "bard_crba_v", "bard_measure_fp32_peak",
            "bard_status_string", "bard_last_error", "bard_launch_count"]
@@ -82,6 +83,7 @@ def lib():
         L.bard_rnea_vjp_workspace_floats.argtypes = [vp, i64]
         L.bard_rnea_vjp_workspace_floats.restype = C.c_size_t
         L.bard_rnea_vjp_params.argtypes = [vp, i64, fp, fp, fp, fp, fp, fp, vp]
+        L.bard_rnea_vjp_params_static.argtypes = [vp, i64, fp, fp, fp, fp, fp, vp]
         L.bard_model_inertial_params.argtypes = [vp, C.POINTER(C.c_double)]
         L.bard_model_set_inertial_params.argtypes = [vp, C.POINTER(C.c_double)]
         L.bard_model_specialize_variant.argtypes = [vp, C.c_uint32, C.c_int, C.c_int]
@@ -290,6 +292,11 @@ class Model:
         """dparams[nb, 10] = sum_b (d tau_b / d theta)^T dtau_b (``bard_rnea_vjp_params``), theta = (m, m c, Io) per link."""
         _check(lib().bard_rnea_vjp_params(self._h, int(B), _ptr(q), _ptr(qd), _ptr(qdd), _ptr(dtau), _ptr(dparams),
                                           _ptr(workspace), stream or None))
+
+    def rnea_vjp_params_static(self, B, q, qd, qdd, dtau, dparams, stream=0):
+        """``bard_rnea_vjp_params_static``: the same with the library's static scratch array (no allocation; calls that
+        overlap on the GPU race on it; refused above ``VJP_STATIC_SCRATCH_FLOATS`` floats of scratch)."""
+        _check(lib().bard_rnea_vjp_params_static(self._h, int(B), _ptr(q), _ptr(qd), _ptr(qdd), _ptr(dtau), _ptr(dparams), stream or None))
 
     def inertial_params(self) -> np.ndarray:
         out = np.zeros((self.nb, 10))

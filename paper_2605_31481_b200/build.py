@@ -12,7 +12,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 LIB = os.path.join(_HERE, "libbard.so")
-SOURCES = ["api.cu", "model.cu", "kernels.cu", "specialize.cu", "vjp.cu", "microbench.cu", "layout.cu", "aba_generic.cu"]
+SOURCES = ["api.cu", "model.cu", "kernels.cu", "specialize.cu", "vjp.cu", "vjp_static.cu", "microbench.cu", "layout.cu", "aba_generic.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC"]
 

@@ -485,6 +485,22 @@ bard_status bard_rnea_vjp_params(const bard_model* bm, int64_t B, const float* q
   return bard::launch_rnea_vjp(bm->m, B, q, qd, qdd, dtau, dparams, workspace, stream);
 }
 
+bard_status bard_rnea_vjp_params_static(const bard_model* bm, int64_t B, const float* q, const float* qd, const float* qdd, const float* dtau,
+                                        float* dparams, bard_stream stream) {
+  if (!bm) { set_error("bard_rnea_vjp_params_static: model is NULL"); return BARD_ERR_INVALID_ARG; }
+  if (!dparams) { set_error("bard_rnea_vjp_params_static: dparams is NULL"); return BARD_ERR_INVALID_ARG; }
+  bard_status s = check_call("bard_rnea_vjp_params_static", bm, B, bm->m.nq ? (const void*)q : dparams, bm->m.nv ? (const void*)qd : dparams,
+                             bm->m.nv ? (const void*)qdd : dparams, bm->m.nv ? (const void*)dtau : dparams);
+  if (s != BARD_OK) return s;
+  bard::DeviceGuard guard(bm->m.device);
+  if (B == 0) {                                             // the sum over no environments
+    cudaError_t e = cudaMemsetAsync(dparams, 0, sizeof(float) * 10 * (size_t)bm->m.nb, (cudaStream_t)stream);
+    if (e != cudaSuccess) { set_error(std::string("bard_rnea_vjp_params_static: ") + cudaGetErrorString(e)); cudaGetLastError(); return BARD_ERR_CUDA; }
+    return BARD_OK;
+  }
+  return bard::launch_rnea_vjp_static(bm->m, B, q, qd, qdd, dtau, dparams, stream);
+}
+
 bard_status bard_model_inertial_params(const bard_model* bm, double* host_params) {
   if (!bm || !host_params) { set_error("bard_model_inertial_params: NULL argument"); return BARD_ERR_INVALID_ARG; }
   for (int i = 0; i < bm->m.nb; ++i)

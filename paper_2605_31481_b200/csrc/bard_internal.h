@@ -237,5 +237,8 @@ size_t rnea_vjp_workspace_floats(const Model& M, int64_t B);
 bard_status launch_rnea_vjp(const Model& M, int64_t B, const float* q, const float* qd, const float* qdd, const float* dtau,
                             float* dparams, float* ws, void* stream);
 bard_status launch_aba(const Model& M, int64_t B, const float* q, const float* qd, const float* tau, float* qdd, float* ws, void* stream);
+// vjp_static.cu: launch_rnea_vjp with the library's static scratch array (no allocation; one array per device, shared)
+bard_status launch_rnea_vjp_static(const Model& M, int64_t B, const float* q, const float* qd, const float* qdd, const float* dtau,
+                                   float* dparams, void* stream);
 
 }  // namespace bard
