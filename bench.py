@@ -388,7 +388,7 @@ def run_only(args):
         k, v = kv.split("=")
         m.set_option(k, int(v))
     if not args.no_specialize:
-        m.specialize(SPEC_OPS + (("aba",) if args.only == "aba" else ()))
+        m.specialize(SPEC_OPS + (("aba",) if args.only == "aba" else ()) + (("rnea_vjp",) if args.only == "vjp" else ()))
     B = args.B
     sets, _ = make_sets(torch, m, desc, args.config, B, dev)
     stream = torch.cuda.current_stream().cuda_stream
@@ -740,14 +740,24 @@ def extras_section(torch, binding, m, desc, cfg, B, dev, stream, pk, spec_s):
         del ws, qdd_out
     except Exception as ex:
         out["aba"] = {"error": str(ex)[:200]}
-    try:    # reverse-mode RNEA w.r.t. the inertial parameters: 4 input arrays, one outward pass
+    try:    # reverse-mode RNEA w.r.t. the inertial parameters: 4 input arrays, one outward pass, the batch sum
         ws = torch.empty(max(1, m.rnea_vjp_workspace_floats(B)), device=dev)
         g = torch.empty((m.nb, 10), device=dev)
-        sec = timed(lambda i: m.rnea_vjp_params(B, sets[i % len(sets)].q, sets[i % len(sets)].qd, sets[i % len(sets)].qdd,
-                                                sets[i % len(sets)].tau, g, ws, stream))
-        io = 4 * (m.nq + 3 * m.nv)
-        out["rnea_vjp"] = {"us": sec * 1e6, "env_evals_per_s": B / sec, "hbm_gbs": io * B / sec / 1e9, "bytes_per_env": io,
-                           "frac_of_hbm": io * B / sec / 1e9 / pk["hbm_gbs"], "launches": 2}
+
+        def vjp(i):
+            x = sets[i % len(sets)]
+            m.rnea_vjp_params(B, x.q, x.qd, x.qdd, x.tau, g, ws, stream)
+        m.set_option("spec_vjp_min_b", 1 << 40)
+        sec_table = timed(vjp)
+        t0 = time.perf_counter()
+        m.specialize(("rnea_vjp",))
+        spec_s["rnea_vjp:" + desc.name] = time.perf_counter() - t0
+        m.set_option("spec_vjp_min_b", -1)
+        sec = timed(vjp)
+        r = op_report(desc, pk, "rnea_vjp", sec, B)
+        out["rnea_vjp"] = {"us": sec * 1e6, "env_evals_per_s": B / sec, "roofline": short(r, ("bound", "achieved", "peak", "unit", "frac")),
+                           "bytes_per_env": r["bytes_per_env"], "flop_per_env": r["flop_per_env"], "hbm_gbs": r["hbm_gbs"], "launches": 2,
+                           "kernel": "bard_rnea_vjp_n1 (generated) + vjp_reduce_columns_kernel", "table_driven_us": sec_table * 1e6}
         del ws, g
     except Exception as ex:
         out["rnea_vjp"] = {"error": str(ex)[:200]}

@@ -21,7 +21,7 @@ BARD_OK = 0
 STATUS = {0: "BARD_OK", 1: "BARD_ERR_INVALID_ARG", 2: "BARD_ERR_TOPOLOGY", 3: "BARD_ERR_UNSUPPORTED",
           4: "BARD_ERR_ALLOC", 5: "BARD_ERR_CUDA"}
 VJP_STATIC_SCRATCH_FLOATS = 262144      # BARD_VJP_STATIC_SCRATCH_FLOATS in include/bard.h
-OPS = {"fk": 1, "jacobian": 2, "rnea": 4, "crba": 8, "fused": 16, "aba": 32, "rnea_roles": 64, "crba_roles": 128, "rnea_pack2": 256, "kin": 512}
+OPS = {"fk": 1, "jacobian": 2, "rnea": 4, "crba": 8, "fused": 16, "aba": 32, "rnea_roles": 64, "crba_roles": 128, "rnea_pack2": 256, "kin": 512, "rnea_vjp": 1024}
 DTYPES = {"f32": 0, "f64": 1}
 LAYOUTS = {"soa": 0, "aos": 1}
 TABLES = {"LEVEL_PTR": (0, np.int32), "LEVEL_BODY": (1, np.int32), "BODY_LEVEL": (2, np.int32),

@@ -132,6 +132,7 @@ struct Specialized;           // specialize.cu: model-specialised (NVRTC) kernel
   X(spec_ldnc, 1)              /* non-coherent (ld.global.nc) input loads in the generated kernels; 0 = coherent */ \
   X(spec_max_block, 512)       /* __launch_bounds__ of the generated kernels (448: 144 registers instead of 128) */ \
   X(spec_solo_smem, 1)         /* one-wave launches ask for > half of the shared memory: one CTA per SM also under PDL */ \
+  X(spec_vjp_min_b, -1)        /* smallest batch for the generated RNEA VJP kernel (auto: 0) */                \
   X(spec_kin, 1)               /* build the kinematics-fused kernel (FK + Jacobian + CRBA) with BARD_OP_FUSED */ \
   X(spec_classical, 1)         /* RNEA of simple models in the classical Newton-Euler form about the COM (fewer FLOPs) */ \
   X(spec_pack, 1)              /* RNEA: 2 = also build the kernel with two environments per thread (FFMA2); it loses: off */ \
@@ -237,6 +238,10 @@ size_t rnea_vjp_workspace_floats(const Model& M, int64_t B);
 bard_status launch_rnea_vjp(const Model& M, int64_t B, const float* q, const float* qd, const float* qdd, const float* dtau,
                             float* dparams, float* ws, void* stream);
 bard_status launch_aba(const Model& M, int64_t B, const float* q, const float* qd, const float* tau, float* qdd, float* ws, void* stream);
+// the generated VJP kernel (specialize.cu) and the sum over its CTAs' columns, partials[np][ncta] (vjp.cu)
+bool launch_vjp_specialized(const Model& M, int64_t B, const float* q, const float* qd, const float* qdd, const float* dtau,
+                            float* dparams, float* ws, void* stream, bard_status& st);
+bard_status launch_vjp_reduce_columns(const float* partials, int ncta, int np, float* dparams, void* stream);
 // vjp_static.cu: launch_rnea_vjp with the library's static scratch array (no allocation; one array per device, shared)
 bard_status launch_rnea_vjp_static(const Model& M, int64_t B, const float* q, const float* qd, const float* qdd, const float* dtau,
                                    float* dparams, void* stream);

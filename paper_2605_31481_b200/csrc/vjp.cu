@@ -178,6 +178,19 @@ __global__ void vjp_reduce_kernel(const float* __restrict__ partials, int nparts
   out[k] = (float)s;
 }
 
+// partials[np][ncta] (the generated kernel's layout): one warp per output, lanes over the CTAs in fp64, fixed order
+__global__ void vjp_reduce_columns_kernel(const float* __restrict__ partials, int ncta, int np, float* __restrict__ out) {
+  const int k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (k >= np) return;
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  const float* p = partials + (size_t)k * ncta;
+  double s = 0.0;
+  for (int c = lane; c < ncta; c += 32) s += (double)p[c];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+  if (lane == 0) out[k] = (float)s;
+}
+
 constexpr size_t kSmemCap = 227 * 1024;
 
 int vjp_grid(const Model& M, int64_t B, int block) {
@@ -195,16 +208,34 @@ int vjp_block(const Model& M, int nslots) {
 
 }  // namespace
 
+// nb * 10 partial sums per CTA; neither kernel (this file's, the generated one of specialize.cu) runs more than
+// min(tiles of 32 environments, 4 CTAs per SM) CTAs, so the size does not depend on which of them serves the call
 size_t rnea_vjp_workspace_floats(const Model& M, int64_t B) {
   if (B <= 0) return 0;
-  const DfsPlan P = dfs_plan(M);
-  const int block = std::max(32, vjp_block(M, P.nslots));
-  return (size_t)vjp_grid(M, B, block) * (size_t)M.nb * 10;
+  return (size_t)vjp_grid(M, B, 32) * (size_t)M.nb * 10;
+}
+
+bard_status launch_vjp_reduce_columns(const float* partials, int ncta, int np, float* dparams, void* stream) {
+  cudaLaunchConfig_t lc = {};
+  lc.gridDim = dim3((unsigned)((np + 3) / 4));
+  lc.blockDim = dim3(128);
+  lc.stream = (cudaStream_t)stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  lc.attrs = attr;
+  lc.numAttrs = 1;
+  const cudaError_t e = cudaLaunchKernelEx(&lc, vjp_reduce_columns_kernel, partials, ncta, np, dparams);
+  if (e != cudaSuccess) { set_error(std::string("bard_rnea_vjp_params: ") + cudaGetErrorString(e)); cudaGetLastError(); return BARD_ERR_CUDA; }
+  g_launches.fetch_add(1);
+  return BARD_OK;
 }
 
 bard_status launch_rnea_vjp(const Model& M, int64_t B, const float* q, const float* qd, const float* qdd, const float* dtau,
                             float* dparams, float* ws, void* stream) {
   if ((int64_t)std::max(M.nq, M.nv) * B >= ((int64_t)1 << 32)) { set_error("bard_rnea_vjp_params: an input array has 2^32 elements or more"); return BARD_ERR_UNSUPPORTED; }
+  bard_status st = BARD_OK;
+  if (launch_vjp_specialized(M, B, q, qd, qdd, dtau, dparams, ws, stream, st)) return st;
   const DfsPlan P = dfs_plan(M);
   const int block = vjp_block(M, P.nslots);
   if (!block) { set_error("bard_rnea_vjp_params: per-environment state does not fit in shared memory"); return BARD_ERR_UNSUPPORTED; }

@@ -5,7 +5,7 @@
 //
 // * Size: BARD_VJP_STATIC_SCRATCH_FLOATS floats = 1 MiB, held by every GPU that loads the library until the process
 //   exits.  A call whose bard_rnea_vjp_workspace_floats(model, B) exceeds it is refused (BARD_ERR_UNSUPPORTED); on a
-//   148-SM part that is a model of more than 44 bodies at a batch of more than ~37 000 environments.
+//   148-SM part that is a model of more than 44 bodies at a batch of more than ~18 600 environments.
 // * In host code the array's NAME is a host-side stand-in, not a device address.  The device address is looked up once
 //   per device, with that device current, by cudaGetSymbolAddress -- in this file, because the array is static -- and
 //   that pointer is what the kernels get.

@@ -119,6 +119,20 @@ def counts(desc) -> dict:
             aba += xform(jt[i]) + (0 if root else 48 + 24) + 72 + (66 + 5 + 6 if has_dof else 0)
             aba += (0 if root else (48 if has_dof else 0) + 78 + 336 + 42 + 27) + (48 + (13 + 6 if has_dof else 0))
 
+    # RNEA VJP w.r.t. the inertial parameters, one outward pass, per body: joint transform; X_up on v, a and
+    # the pushed cotangent lambda (42 each: R^T w 15, w x t 9, + 3, R^T (.) 15); S qd, S qdd, S dtau and their adds (36);
+    # a += v x S qd (36); u = v x lambda (30); the ten bilinear terms (86: m 11, h 45, Io 30); the batch sum (10).
+    # Root bodies: v = S qd, a = R^T (-g) + S qdd, lambda = S dtau.  Free joints: the joint vectors are the inputs themselves.
+    vjp = 0
+    for i in range(nb):
+        root = parent[i] < 0
+        if jt[i] == FREE:
+            vjp += 36 + (18 if root else 126 + 18 + 36) + 30 + 86 + 10
+        elif jt[i] == FIXED:
+            vjp += (15 if root else 126) + 30 + 86 + 10
+        else:
+            vjp += xform(jt[i]) + (36 if root else 126 + 36 + 36) + 30 + 86 + 10
+
     def row(i, o, f):
         return {"in": i, "out": o, "bytes": i + o, "flop": f}
 
@@ -128,6 +142,7 @@ def counts(desc) -> dict:
         "rnea": row(4 * (nq + 2 * nv), 4 * nv, rnea),
         "crba": row(4 * nq, 4 * nv * nv, crba),
         "aba": row(4 * (nq + 2 * nv), 4 * nv, aba),
+        "rnea_vjp": row(4 * (nq + 3 * nv), 0, vjp),
         # bard_kinematics: q read once; FK is part of CRBA's walk, the Jacobian adds its axis and column work
         "kin": row(4 * nq, 48 * nb + 24 * nf * nv + 4 * nv * nv, crba + jac - sum(xform(jt[i]) + (63 if parent[i] >= 0 else 0) for i in used)),
     }

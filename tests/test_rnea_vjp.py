@@ -171,6 +171,35 @@ def test_gpu_vjp_matches_oracle(idx, B):
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("idx", range(8))
+@pytest.mark.parametrize("B", [1, 37, 1000, 4096 + 17, 200003])
+def test_gpu_generated_vjp_matches_oracle_and_table_kernel(idx, B):
+    """bard_model_specialize(BARD_OP_RNEA_VJP): the generated kernel (one tile per CTA up to one wave, a grid-stride loop
+    over tiles beyond: 200 003, ragged) against the oracle, against the table-driven kernel, and bit-identical on a repeat."""
+    desc = _robots()[idx]
+    m = binding.Model(desc, device=0)
+    o = oracle.Oracle(desc)
+    q, qd, qdd = W.sample_states(desc, B, seed=151 + idx)
+    dtau = np.random.default_rng(idx).normal(size=(desc.nv, B)).astype(np.float32)
+    g_table = gpu_vjp(m, q, qd, qdd, dtau)
+    m.specialize(("rnea_vjp",))
+    assert "bard_rnea_vjp_n1" in m.specialized_source("rnea_vjp")
+    n0 = binding.launch_count()
+    g1, g2 = gpu_vjp(m, q, qd, qdd, dtau, repeat=2)
+    assert binding.launch_count() - n0 == 4                                  # the generated kernel + the sum over its CTAs, twice
+    assert np.isfinite(g1).all()
+    assert np.array_equal(g1, g2)
+    if B <= 5000:                                                            # the oracle needs nb * 10 RNEAs per environment
+        ref = o.rnea_vjp_params(*(a.astype(np.float64) for a in (q, qd, qdd, dtau)))
+        assert nerr(g1, ref) <= TOL
+    else:                                                                    # the whole batch: against the table-driven kernel (itself held to the oracle)
+        scale = np.maximum(1.0, np.abs(g_table.astype(np.float64)))
+        assert float(np.max(np.abs(g1.astype(np.float64) - g_table) / scale)) <= TOL * max(1.0, np.sqrt(B / 4096.0))
+    m.set_option("spec_vjp_min_b", 1 << 40)                                  # the table-driven kernel again
+    assert np.array_equal(gpu_vjp(m, q, qd, qdd, dtau), g_table)
+
+
+@pytest.mark.gpu
 def test_gpu_vjp_full_size_and_adjoint_identity():
     """Humanoid at B = 65 536 (bench size): against the oracle's definition (240 RNEA evaluations per environment on the
     host cores), and the adjoint identity dparams . dtheta = sum dtau . tau(dtheta) with tau(dtheta) from the GPU's own
