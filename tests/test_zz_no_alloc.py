@@ -24,11 +24,13 @@ def _inputs(desc, B, seed, dev):
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("cfg", [0, 3])
-def test_static_scratch_vjp_matches_the_workspace_path_on_two_calls_in_a_row(cfg):
+@pytest.mark.parametrize("cfg,generated", [(0, False), (3, False), (3, True)])
+def test_static_scratch_vjp_matches_the_workspace_path_on_two_calls_in_a_row(cfg, generated):
     dev = torch.device("cuda:0")
     desc = W.config_robot(cfg)
     m = binding.Model(desc, device=0)
+    if generated:
+        m.specialize(("rnea_vjp",))          # both entry points then run the generated kernel
     stream = torch.cuda.current_stream().cuda_stream
     # two different calls in a row on one stream: a large batch (every CTA's partials used), then a small ragged one (the
     # array still holds the first call's partials beyond the second call's grid: they must not be read)
