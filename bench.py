@@ -12,7 +12,8 @@ Besides the headline the default run (rank 0, one GPU) reports, compactly:
   * ``matrix``: every operator and bard_step on configs 0-3 at B = 4096 and 65 536 (BASELINE.json's metric);
   * ``sweep``: BASELINE.json config 4 -- humanoid and chain-7 at B = 1024 ... 1 048 576: env-evals/s, achieved HBM GB/s
     and FP32 TFLOP/s against the B200 peaks, and the oracle's time on the host cores per B;
-  * ``aba`` (with its roofline), ``rnea_vjp``, ``variants`` (fp64 / AoS), ``config2_rollout``, ``specialize_s``.
+  * ``aba`` and ``rnea_vjp`` (generated kernels, each with its roofline; the VJP also table-driven), ``variants``
+    (fp64 / AoS), ``config2_rollout``, ``specialize_s``.
 Per-operator times are device times of a back-to-back train of launches over rotating buffer sets (> L2 in total)
 replayed from a CUDA graph, so that a kernel shorter than the host's launch rate is timed as a kernel.
 
