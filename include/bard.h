@@ -165,7 +165,7 @@ bard_status bard_crba(const bard_model* m, int64_t B, const float* q, float* M, 
 
 /* The three operators that depend on q alone -- poses, Jacobians and the mass matrix -- of one batch.  They share joint
  * transforms, world poses and screws (the paper's tiered cache: one FK evaluation shared by the queries): if
- * the model was specialised with BARD_OP_FUSED and B > 256 x SM count, ONE kernel walks the tree once and stores all three
+ * the model was specialised with BARD_OP_FUSED and B is above bard_step's fork regime (below), ONE kernel walks the tree once and stores all three
  * (the kernel bard_step launches beside bard_rnea on the larger robots); otherwise bard_fk, bard_jacobian and bard_crba in
  * sequence on `stream`.  Outputs and layouts as for the three calls. */
 bard_status bard_kinematics(const bard_model* m, int64_t B, const float* q, float* pose, float* J, float* M, bard_stream stream);
@@ -173,7 +173,7 @@ bard_status bard_kinematics(const bard_model* m, int64_t B, const float* q, floa
 /* One simulation step's worth of operators on one batch: poses, Jacobians, torques and mass matrix of the same
  * (q, qd, qdd) -- the paper's tiered cache and "full pipeline" restated on chip.  The form is chosen
  * per call from the batch size (option step_mode forces one):
- *   B <= step_fork_max_b (256 x SM count): one operator's grid does not fill the machine, so bard_fk, bard_jacobian, bard_rnea and
+ *   B <= step_fork_max_b: one operator's grid does not fill the machine, so bard_fk, bard_jacobian, bard_rnea and
  *     bard_crba are FORKED over three internal side streams and joined back into `stream`: the step costs its longest
  *     operator, not the sum; the fork-join is ordered after everything already in `stream`, is complete before anything
  *     enqueued later, and can be captured into a CUDA graph (one capture at a time per model);
@@ -182,6 +182,13 @@ bard_status bard_kinematics(const bard_model* m, int64_t B, const float* q, floa
  *     or TWO: the kinematics-fused kernel (FK + Jacobian + CRBA in one walk: they share q, poses and screws) and
  *     bard_rnea on an internal side stream (ALU-bound beside an HBM-bound kernel), joined back into `stream`;
  *   otherwise the four operators in sequence on `stream`.
+ * Where the fork regime ends (option step_fork_max_b, -1 = automatic; bard_model_get_option(m, "step_fork_regime", &v) reads the
+ * current answer): 256 x SM count on a model without generated kernels.  bard_model_specialize(model, ... | BARD_OP_FUSED) on a
+ * device model MEASURES it: it times the forked step and the one- / two-launch step at B = 4096 on the model's device (eleven
+ * plain calls each on scratch buffers it allocates and frees: a build-time call) and lets the one- / two-launch form take
+ * over from 3072 environments if it is already faster there (a 7-DOF arm's fused kernel, an 11-DOF spined quadruped: short
+ * walks, and no fork-join on the host), else from 128 x SM count.  Option step_calibrate = 0 replaces the measurement by a
+ * static rule on the length of the generated walk (step_light_max).
  * Outputs and layouts as for the four calls. */
 bard_status bard_step(const bard_model* m, int64_t B, const float* q, const float* qd, const float* qdd,
                       float* pose, float* J, float* tau, float* M, bard_stream stream);

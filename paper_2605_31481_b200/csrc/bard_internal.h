@@ -117,7 +117,9 @@ struct Specialized;           // specialize.cu: model-specialised (NVRTC) kernel
   X(spec_fused_max_rows, 112)  /* the fused step kernel is used at every batch up to this many parked rows */  \
   X(spec_fused_small_b, -1)    /* ... and above it only up to this batch */                                    \
   X(spec_kin_min_b, -1)        /* smallest batch at which bard_step uses the kinematics-fused kernel + RNEA */ \
-  X(step_fork_max_b, -1)       /* bard_step forks the four operators over side streams up to this batch (auto: 256 x SMs) */ \
+  X(step_fork_max_b, -1)       /* bard_step forks the four operators over side streams up to this batch (auto: step_fork_max_b() in specialize.cu) */ \
+  X(step_light_max, 2000)      /* ... not measured: a one-/two-launch step of at most this many arithmetic statements per thread takes over from 3072 environments */ \
+  X(step_calibrate, 1)         /* bard_model_specialize(BARD_OP_FUSED) times the forked and the one-/two-launch step at B = 4096 and sets the fork regime from that */ \
   X(step_kin_fork, 1)          /* bard_step = kinematics-fused kernel + RNEA: RNEA on a side stream (1) or after it (0) */ \
   X(step_mode, -1)             /* bard_step: -1 auto, 0 four launches in sequence, 1 forked, 2 one-launch kernel */ \
   /* read by bard_model_specialize (code generation) */                                                        \
@@ -150,6 +152,7 @@ struct Model {
   int device = 0;
   Options opt;
   Specialized* spec = nullptr;
+  int64_t fork_max_cal = -1;          // bard_step's fork regime as bard_model_specialize measured it (-1: not measured)
   int32_t nb = 0, nq = 0, nv = 0, nlevels = 0, nslots = 0, nframes = 0, nfree = 0;
   int32_t team_warps = 1;             // L: warps that share one 32-environment tile (level-parallel schedule)
   int32_t crba_warps = 1;             // Lc >= L: CRBA adds warps that only join the fill of M
@@ -224,6 +227,7 @@ bard_status launch_f64(const Model& M, uint32_t op, int64_t B, const void* q, co
 // layout.cu: [rows][cols] -> [cols][rows] at HBM speed (elem = 4 or 8 bytes), one launch
 bard_status launch_transpose(const void* src, void* dst, int64_t rows, int64_t cols, int elem, void* stream);
 bool kin_available(const Model& M, int64_t B);
+int64_t step_fork_max_b(const Model& M);
 bool launch_kin(const Model& M, int64_t B, const float* q, float* pose, float* J, float* Mo, void* stream, bard_status& st);
 void drop_specialized_jacobian(Model& M);
 void drop_specialized_dynamics(Model& M);      // kernels with the inertial parameters folded in as literals

@@ -363,7 +363,31 @@ def test_kinematics_fused_step_matches_oracle_and_the_four_kernels(cfg, B, kin_f
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("cfg,B,specialised", [(3, 65536, True), (3, 1000, True), (1, 300, False), (2, 40000, True)])
+def test_step_fork_regime_is_measured_at_specialisation():
+    """Where bard_step stops forking: 256 x SMs without generated kernels; bard_model_specialize(BARD_OP_FUSED) then times
+    both forms at B = 4096 on the device (margins on these two robots: 2x) -- or applies the static rule when told not to
+    measure; an explicit step_fork_max_b always wins; bard_model_set_frames drops the measurement with the kernels."""
+    sms = 148
+    for cfg, want in ((3, 128 * sms), (0, 3072)):
+        desc = W.config_robot(cfg)
+        m = binding.Model(desc, device=0)
+        assert m.get_option("step_fork_regime") == 256 * sms
+        m.specialize(ALL + ("fused",))
+        assert m.get_option("step_fork_regime") == want
+        m.set_option("step_fork_max_b", 1234)
+        assert m.get_option("step_fork_regime") == 1234
+        m.set_option("step_fork_max_b", -1)
+        m.set_frames(desc.frame_body, desc.frame_offset)
+        assert m.get_option("step_fork_regime") in (256 * sms, 128 * sms, 3072)       # the static rule on what is left
+        m2 = binding.Model(desc, device=0)
+        m2.set_option("step_calibrate", 0)
+        m2.specialize(ALL + ("fused",))
+        assert m2.get_option("step_fork_regime") == want                                # the static rule agrees on the BASELINE robots
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("cfg,B,specialised", [(3, 65536, True), (3, 1000, True), (1, 300, False), (2, 40000, True), (2, 5000, True), (2, 3000, True),
+                                               (3, 20000, True), (3, 10000, True)])
 def test_bard_kinematics_matches_oracle(cfg, B, specialised):
     """bard_kinematics: pose, J and M of one batch -- one launch of the kinematics-fused kernel where it exists and the
     batch is in its regime, bard_fk + bard_jacobian + bard_crba otherwise; either way the three operators' results."""
@@ -379,7 +403,8 @@ def test_bard_kinematics_matches_oracle(cfg, B, specialised):
     n0 = binding.launch_count()
     m.kinematics(B, tq, *outs, torch.cuda.current_stream().cuda_stream)
     torch.cuda.synchronize()
-    one = specialised and B > 256 * 148 and "bard_kin_n1" in m.specialized_source("kin") if specialised and cfg != 1 else False
+    # the fork regime of bard_step ends at 3072 environments where the kinematics walk is short (spined quadruped), at 128 x SMs otherwise
+    one = specialised and cfg != 1 and B > (3072 if cfg == 2 else 128 * 148) and "bard_kin_n1" in m.specialized_source("kin")
     assert binding.launch_count() - n0 == (1 if one else 3)
     idx = np.unique(np.concatenate([np.arange(0, B, max(1, B // 400)), [B - 1]]))
     q64 = np.ascontiguousarray(q[:, idx].astype(np.float64))
