@@ -111,6 +111,7 @@ struct Specialized;           // specialize.cu: model-specialised (NVRTC) kernel
   /* which kernel family a call gets (specialize.cu, api.cu) */                                                \
   X(spec_min_b, -1)            /* smallest batch for the plain specialised kernels */                          \
   X(spec_block, 0)             /* force the CTA size of the specialised kernels */                             \
+  X(spec_min_block, -1)        /* smallest CTA of a one-wave launch of the compute-bound generated kernels (-1: per kernel, 256 / 128; 0: off) */ \
   X(spec_roles_max_b, -1)      /* largest batch for the limb-role RNEA */                                      \
   X(spec_crba_roles_max_b, -1) /* largest / smallest batch for the limb-role CRBA */                           \
   X(spec_crba_roles_min_b, -1)                                                                                 \
