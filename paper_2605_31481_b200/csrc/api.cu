@@ -157,45 +157,64 @@ bard_status bard_model_set_frames(bard_model* bm, int32_t nframes, const int32_t
 }
 
 // Which form of bard_step is faster for THIS model on THIS device at a small batch, measured: the forked step and the one-
-// / two-launch step, eight plain calls each at B = 4096 on scratch buffers (zeros; unit quaternions), CUDA events on a
-// stream of its own.  The faster one decides where the fork regime ends (specialize.cu: step_fork_max_b): 3072 if the
-// one- / two-launch form wins already here, 128 x SMs otherwise.  Plain calls on purpose: a caller that does not replay
-// CUDA graphs pays the fork-join's sixteen API calls.  Best effort: any failure leaves the static rule in charge.
+// / two-launch step at B = 4096 on scratch buffers (zeros; unit quaternions), on a stream of its own, timed with CUDA events
+// TWICE: as eight plain calls (a caller that does not replay CUDA graphs pays the fork-join's sixteen API calls: 15-20 us)
+// and as a captured graph of eight calls replayed (device time only).  The faster form decides where the fork regime
+// ends for plain calls and for calls under stream capture respectively (specialize.cu: step_fork_max_b): 3072 if the one-
+// / two-launch form wins already at B = 4096, 8192 if it wins at 16 384 (measured the same way), 128 x SMs otherwise.  Best
+// effort: any failure leaves the static rule in charge.
 static void calibrate_step(bard_model* bm) {
   bard::Model& m = bm->m;
-  m.fork_max_cal = -1;
+  m.fork_max_cal[0] = m.fork_max_cal[1] = -1;
   if (!m.d_blob || m.nv == 0 || m.nframes == 0 || m.opt.step_calibrate == 0 || m.opt.step_fork_max_b >= 0 || !bm->fj.ok) return;
-  const int64_t B = 4096;
-  const size_t n_in = (size_t)(m.nq + 2 * m.nv) * B;
-  const size_t n_pose = (size_t)12 * m.nb * B, n_J = (size_t)6 * m.nframes * m.nv * B, n_tau = (size_t)m.nv * B, n_M = (size_t)m.nv * m.nv * B;
+  const int64_t sizes[2] = {4096, 16384}, Bmax = sizes[1];
+  const size_t n_in = (size_t)(m.nq + 2 * m.nv) * Bmax;
+  const size_t n_out = ((size_t)12 * m.nb + (size_t)6 * m.nframes * m.nv + (size_t)m.nv + (size_t)m.nv * m.nv) * Bmax;
   bard::DeviceGuard guard(m.device);
   float* buf = nullptr;
   cudaStream_t st = nullptr;
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   const int64_t keep_mode = m.opt.step_mode;
-  float t[2] = {0.f, 0.f};
-  bool ok = cudaMalloc(&buf, sizeof(float) * (n_in + n_pose + n_J + n_tau + n_M)) == cudaSuccess &&
+  float t[2][2][2] = {};                             // [batch][plain / graph][forked / not]
+  bool ok = cudaMalloc(&buf, sizeof(float) * (n_in + n_out)) == cudaSuccess &&
             cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) == cudaSuccess && cudaEventCreate(&e0) == cudaSuccess &&
             cudaEventCreate(&e1) == cudaSuccess && cudaMemsetAsync(buf, 0, sizeof(float) * n_in, st) == cudaSuccess;
-  if (ok) {
+  for (int sz = 0; sz < 2 && ok; ++sz) {
+    const int64_t B = sizes[sz];
+    float *q = buf, *qd = buf + (size_t)m.nq * B, *qdd = qd + (size_t)m.nv * B, *pose = buf + n_in, *J = pose + (size_t)12 * m.nb * B,
+          *tau = J + (size_t)6 * m.nframes * m.nv * B, *Mo = tau + (size_t)m.nv * B;
     const std::vector<float> ones((size_t)B, 1.0f);
-    for (int i = 0; i < m.nb && ok; ++i)
+    ok = cudaMemsetAsync(buf, 0, sizeof(float) * n_in, st) == cudaSuccess;
+    for (int i = 0; i < m.nb && ok; ++i)           // unit quaternions
       if (m.jtype[i] == BARD_JOINT_FREE)
-        ok = cudaMemcpyAsync(buf + (size_t)(m.q_off[i] + 6) * B, ones.data(), sizeof(float) * B, cudaMemcpyHostToDevice, st) == cudaSuccess &&
+        ok = cudaMemcpyAsync(q + (size_t)(m.q_off[i] + 6) * B, ones.data(), sizeof(float) * B, cudaMemcpyHostToDevice, st) == cudaSuccess &&
              cudaStreamSynchronize(st) == cudaSuccess;
-  }
-  float *q = buf, *qd = buf + (size_t)m.nq * B, *qdd = qd + (size_t)m.nv * B, *pose = buf + n_in, *J = pose + n_pose, *tau = J + n_J, *Mo = tau + n_tau;
-  for (int form = 0; form < 2 && ok; ++form) {
-    m.opt.step_mode = form == 0 ? 1 : -1;           // forked / whatever follows the fork regime
-    m.fork_max_cal = form == 0 ? -1 : 0;
-    for (int k = 0; k < 11 && ok; ++k) {
-      if (k == 3) ok = cudaEventRecord(e0, st) == cudaSuccess;
-      ok = ok && bard_step(bm, B, q, qd, qdd, pose, J, tau, Mo, st) == BARD_OK;
+    for (int form = 0; form < 2 && ok; ++form) {
+      m.opt.step_mode = form == 0 ? 1 : -1;         // forked / whatever follows the fork regime
+      m.fork_max_cal[0] = m.fork_max_cal[1] = form == 0 ? -1 : 0;
+      for (int k = 0; k < 11 && ok; ++k) {          // plain calls
+        if (k == 3) ok = cudaEventRecord(e0, st) == cudaSuccess;
+        ok = ok && bard_step(bm, B, q, qd, qdd, pose, J, tau, Mo, st) == BARD_OK;
+      }
+      ok = ok && cudaEventRecord(e1, st) == cudaSuccess && cudaStreamSynchronize(st) == cudaSuccess && cudaEventElapsedTime(&t[sz][0][form], e0, e1) == cudaSuccess;
+      cudaGraph_t g = nullptr;                      // the same eight calls as a graph
+      cudaGraphExec_t ge = nullptr;
+      if (ok && cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+        for (int k = 0; k < 8 && ok; ++k) ok = bard_step(bm, B, q, qd, qdd, pose, J, tau, Mo, st) == BARD_OK;
+        ok = (cudaStreamEndCapture(st, &g) == cudaSuccess) && ok && g;
+      } else {
+        ok = false;
+      }
+      ok = ok && cudaGraphInstantiate(&ge, g, 0) == cudaSuccess && cudaGraphLaunch(ge, st) == cudaSuccess && cudaEventRecord(e0, st) == cudaSuccess &&
+           cudaGraphLaunch(ge, st) == cudaSuccess && cudaGraphLaunch(ge, st) == cudaSuccess && cudaEventRecord(e1, st) == cudaSuccess &&
+           cudaStreamSynchronize(st) == cudaSuccess && cudaEventElapsedTime(&t[sz][1][form], e0, e1) == cudaSuccess;
+      if (ge) cudaGraphExecDestroy(ge);
+      if (g) cudaGraphDestroy(g);
     }
-    ok = ok && cudaEventRecord(e1, st) == cudaSuccess && cudaStreamSynchronize(st) == cudaSuccess && cudaEventElapsedTime(&t[form], e0, e1) == cudaSuccess;
   }
   m.opt.step_mode = keep_mode;
-  m.fork_max_cal = ok ? (t[1] < t[0] ? 96 * 32 : 128 * (int64_t)m.sm_count) : -1;
+  for (int how = 0; how < 2; ++how)
+    m.fork_max_cal[how] = !ok ? -1 : t[0][how][1] < t[0][how][0] ? 96 * 32 : t[1][how][1] < t[1][how][0] ? 8192 : 128 * (int64_t)m.sm_count;
   if (!ok) cudaGetLastError();
   if (e0) cudaEventDestroy(e0);
   if (e1) cudaEventDestroy(e1);
@@ -220,7 +239,8 @@ bard_status bard_model_set_option(bard_model* bm, const char* key, int64_t value
 
 bard_status bard_model_get_option(const bard_model* bm, const char* key, int64_t* value) {
   if (!bm || !value) { set_error("bard_model_get_option: NULL argument"); return BARD_ERR_INVALID_ARG; }
-  if (key && std::strcmp(key, "step_fork_regime") == 0) { *value = bard::step_fork_max_b(bm->m); return BARD_OK; }   // read-only: the rule's current answer
+  if (key && std::strcmp(key, "step_fork_regime") == 0) { *value = bard::step_fork_max_b(bm->m, false); return BARD_OK; }   // read-only: the rule's current answer
+  if (key && std::strcmp(key, "step_fork_regime_captured") == 0) { *value = bard::step_fork_max_b(bm->m, true); return BARD_OK; }
   int64_t* ref = nullptr;
   if (!bard::option_ref(const_cast<bard_model*>(bm)->m.opt, key, &ref)) { set_error(std::string("bard_model_get_option: unknown option: ") + (key ? key : "(null)")); return BARD_ERR_INVALID_ARG; }
   *value = *ref;
@@ -315,7 +335,9 @@ bard_status bard_step(const bard_model* bm, int64_t B, const float* q, const flo
   //    else the four operators in sequence on the caller's stream.
   // step_mode forces a form (tests, experiments).
   const int64_t mode = bm->m.opt.step_mode;
-  const int64_t fork_max_b = bard::step_fork_max_b(bm->m);
+  cudaStreamCaptureStatus capture = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing((cudaStream_t)stream, &capture) != cudaSuccess) { cudaGetLastError(); capture = cudaStreamCaptureStatusNone; }
+  const int64_t fork_max_b = bard::step_fork_max_b(bm->m, capture == cudaStreamCaptureStatusActive);
   StepFork& f = const_cast<bard_model*>(bm)->fj;
   const bool want_fork = mode == 1 || (mode < 0 && B <= fork_max_b);
   if (bm->m.nv > 0 && bm->m.nframes > 0 && (mode == 2 || (mode < 0 && !want_fork))) {

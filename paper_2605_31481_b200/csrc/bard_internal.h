@@ -153,7 +153,7 @@ struct Model {
   int device = 0;
   Options opt;
   Specialized* spec = nullptr;
-  int64_t fork_max_cal = -1;          // bard_step's fork regime as bard_model_specialize measured it (-1: not measured)
+  int64_t fork_max_cal[2] = {-1, -1}; // bard_step's fork regime as bard_model_specialize measured it (-1: not measured): [0] plain calls, [1] under stream capture
   int32_t nb = 0, nq = 0, nv = 0, nlevels = 0, nslots = 0, nframes = 0, nfree = 0;
   int32_t team_warps = 1;             // L: warps that share one 32-environment tile (level-parallel schedule)
   int32_t crba_warps = 1;             // Lc >= L: CRBA adds warps that only join the fill of M
@@ -228,7 +228,7 @@ bard_status launch_f64(const Model& M, uint32_t op, int64_t B, const void* q, co
 // layout.cu: [rows][cols] -> [cols][rows] at HBM speed (elem = 4 or 8 bytes), one launch
 bard_status launch_transpose(const void* src, void* dst, int64_t rows, int64_t cols, int elem, void* stream);
 bool kin_available(const Model& M, int64_t B);
-int64_t step_fork_max_b(const Model& M);
+int64_t step_fork_max_b(const Model& M, bool capturing);
 bool launch_kin(const Model& M, int64_t B, const float* q, float* pose, float* J, float* Mo, void* stream, bard_status& st);
 void drop_specialized_jacobian(Model& M);
 void drop_specialized_dynamics(Model& M);      // kernels with the inertial parameters folded in as literals
