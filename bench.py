@@ -458,6 +458,9 @@ def run_ours(args):
         if c not in models:
             d = W.config_robot(c)
             mm = binding.Model(d, device=local)
+            for kv in args.option:                      # experiments: bard_model_set_option before specialising
+                k, v = kv.split("=")
+                mm.set_option(k, int(v))
             if not args.no_specialize:
                 t0 = time.perf_counter()
                 mm.specialize(SPEC_OPS)

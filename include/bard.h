@@ -185,12 +185,12 @@ bard_status bard_kinematics(const bard_model* m, int64_t B, const float* q, floa
  * Where the fork regime ends (option step_fork_max_b, -1 = automatic; bard_model_get_option(m, "step_fork_regime" /
  * "step_fork_regime_captured", &v) reads the current answer for plain calls / calls under stream capture): 256 x SM count on
  * a model without generated kernels.  bard_model_specialize(model, ... | BARD_OP_FUSED) on a device model MEASURES it: it times
- * the forked step and the one- / two-launch step at B = 4096 and 16 384 on the model's device, as plain calls and as a
- * captured graph replayed (scratch buffers it allocates and frees: a build-time call, a few ms), and lets the one- / two-launch
- * form take over from 3072 environments if it is already faster at 4096 (as plain calls: a 7-DOF arm's fused kernel, an
- * 11-DOF spined quadruped -- short walks, and no fork-join on the host: sixteen API calls), from 8192 if it is faster at
- * 16 384, else from 128 x SM count; bard_step asks the stream whether it is being captured (cudaStreamIsCapturing) and uses the
- * matching answer.  Option step_calibrate = 0 replaces the measurement by a static rule on the length of the generated walk
+ * the forked step and the one- / two-launch step at B = 4096 and 16 384 on the model's device as plain calls (scratch buffers
+ * it allocates and frees: a build-time call, a few ms) and lets the one- / two-launch form take over from 3072 environments
+ * if it is already faster at 4096 (a 7-DOF arm's fused kernel, an 11-DOF spined quadruped -- short walks, and no fork-join on
+ * the host: sixteen API calls), from 8192 if it is faster at 16 384, else from 128 x SM count.  Under stream capture the host
+ * cost does not exist and forking pays a little longer: bard_step asks the stream (cudaStreamIsCapturing) and then forks up
+ * to at least 8192.  Option step_calibrate = 0 replaces the measurement by a static rule on the length of the generated walk
  * (step_light_max).
  * Outputs and layouts as for the four calls. */
 bard_status bard_step(const bard_model* m, int64_t B, const float* q, const float* qd, const float* qdd,

@@ -156,13 +156,16 @@ bard_status bard_model_set_frames(bard_model* bm, int32_t nframes, const int32_t
   return bard::set_frames(bm->m, nframes, body, offset);
 }
 
-// Which form of bard_step is faster for THIS model on THIS device at a small batch, measured: the forked step and the one-
-// / two-launch step at B = 4096 on scratch buffers (zeros; unit quaternions), on a stream of its own, timed with CUDA events
-// TWICE: as eight plain calls (a caller that does not replay CUDA graphs pays the fork-join's sixteen API calls: 15-20 us)
-// and as a captured graph of eight calls replayed (device time only).  The faster form decides where the fork regime
-// ends for plain calls and for calls under stream capture respectively (specialize.cu: step_fork_max_b): 3072 if the one-
-// / two-launch form wins already at B = 4096, 8192 if it wins at 16 384 (measured the same way), 128 x SMs otherwise.  Best
-// effort: any failure leaves the static rule in charge.
+// Which form of bard_step is faster for THIS model on THIS device at small batches, measured: the forked step and the one-
+// / two-launch step at B = 4096 and 16 384 on scratch buffers (zeros; unit quaternions), eight plain calls each on a stream
+// of its own between CUDA events -- plain calls on purpose: a caller that does not replay CUDA graphs pays the fork-join's
+// sixteen API calls (15-20 us).  The faster form decides where the fork regime ends (specialize.cu: step_fork_max_b): 3072
+// if the one- / two-launch form wins already at 4096, 8192 if it wins at 16 384, 128 x SMs otherwise.  Under stream capture
+// the host cost does not exist and forking pays a little longer: where the plain-call answer is below 8192 the captured
+// one is 8192 (graph replay on the four robots: spined quadruped at 4096 / 8192 forked 10.8 / 10.8 us, fused 13.1 / 13.1; at
+// 12 288 13.1 / 13.3; chain-7 6.2-6.9 / 6.9).  That second answer is a rule, not a measurement, because measuring it means
+// building a CUDA graph here, and a process that has launched one ran the humanoid's 65 536-environment step 3 % slower
+// afterwards (96.7 against 93.6 us, reproducibly).  Best effort: any failure leaves the static rule in charge.
 static void calibrate_step(bard_model* bm) {
   bard::Model& m = bm->m;
   m.fork_max_cal[0] = m.fork_max_cal[1] = -1;
@@ -175,7 +178,7 @@ static void calibrate_step(bard_model* bm) {
   cudaStream_t st = nullptr;
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   const int64_t keep_mode = m.opt.step_mode;
-  float t[2][2][2] = {};                             // [batch][plain / graph][forked / not]
+  float t[2][2] = {};                                // [batch][forked / not]
   bool ok = cudaMalloc(&buf, sizeof(float) * (n_in + n_out)) == cudaSuccess &&
             cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) == cudaSuccess && cudaEventCreate(&e0) == cudaSuccess &&
             cudaEventCreate(&e1) == cudaSuccess && cudaMemsetAsync(buf, 0, sizeof(float) * n_in, st) == cudaSuccess;
@@ -196,25 +199,12 @@ static void calibrate_step(bard_model* bm) {
         if (k == 3) ok = cudaEventRecord(e0, st) == cudaSuccess;
         ok = ok && bard_step(bm, B, q, qd, qdd, pose, J, tau, Mo, st) == BARD_OK;
       }
-      ok = ok && cudaEventRecord(e1, st) == cudaSuccess && cudaStreamSynchronize(st) == cudaSuccess && cudaEventElapsedTime(&t[sz][0][form], e0, e1) == cudaSuccess;
-      cudaGraph_t g = nullptr;                      // the same eight calls as a graph
-      cudaGraphExec_t ge = nullptr;
-      if (ok && cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
-        for (int k = 0; k < 8 && ok; ++k) ok = bard_step(bm, B, q, qd, qdd, pose, J, tau, Mo, st) == BARD_OK;
-        ok = (cudaStreamEndCapture(st, &g) == cudaSuccess) && ok && g;
-      } else {
-        ok = false;
-      }
-      ok = ok && cudaGraphInstantiate(&ge, g, 0) == cudaSuccess && cudaGraphLaunch(ge, st) == cudaSuccess && cudaEventRecord(e0, st) == cudaSuccess &&
-           cudaGraphLaunch(ge, st) == cudaSuccess && cudaGraphLaunch(ge, st) == cudaSuccess && cudaEventRecord(e1, st) == cudaSuccess &&
-           cudaStreamSynchronize(st) == cudaSuccess && cudaEventElapsedTime(&t[sz][1][form], e0, e1) == cudaSuccess;
-      if (ge) cudaGraphExecDestroy(ge);
-      if (g) cudaGraphDestroy(g);
+      ok = ok && cudaEventRecord(e1, st) == cudaSuccess && cudaStreamSynchronize(st) == cudaSuccess && cudaEventElapsedTime(&t[sz][form], e0, e1) == cudaSuccess;
     }
   }
   m.opt.step_mode = keep_mode;
-  for (int how = 0; how < 2; ++how)
-    m.fork_max_cal[how] = !ok ? -1 : t[0][how][1] < t[0][how][0] ? 96 * 32 : t[1][how][1] < t[1][how][0] ? 8192 : 128 * (int64_t)m.sm_count;
+  m.fork_max_cal[0] = !ok ? -1 : t[0][1] < t[0][0] ? 96 * 32 : t[1][1] < t[1][0] ? 8192 : 128 * (int64_t)m.sm_count;
+  m.fork_max_cal[1] = !ok ? -1 : std::max<int64_t>(m.fork_max_cal[0], 8192);
   if (!ok) cudaGetLastError();
   if (e0) cudaEventDestroy(e0);
   if (e1) cudaEventDestroy(e1);
