@@ -139,7 +139,8 @@ enum { BARD_OP_FK = 1, BARD_OP_JACOBIAN = 2, BARD_OP_RNEA = 4, BARD_OP_CRBA = 8,
  * inward pass of a subtree follows its outward pass (eq. (6)) and only the bodies on
  * the current root-to-leaf path hold parked state -- compiles it for sm_100a with NVRTC (libnvrtc.so.12 of the
  * CUDA toolkit, loaded with dlopen) and loads the cubin.  Afterwards bard_<op> calls with a large batch
- * launch the specialised kernel (chains: any B; teams of <= 4 warps: B >= 4096; wider: B >= 32768), smaller ones
+ * launch the specialised kernel (thresholds measured per operator -- chains: any B; teams of <= 4 warps: FK / Jacobian any B,
+ * RNEA / CRBA B >= 4096; wider teams: Jacobian B >= 5000, FK B >= 16385, CRBA B >= 18945, RNEA B >= 32768), smaller ones
  * the level-parallel team kernel; results agree to rounding.  BARD_OP_RNEA on a single-rooted tree that branches
  * also builds a limb-role RNEA kernel (the subtrees below the first branching body dealt to two groups of warps
  * of the CTA, siblings' forces summed in ascending child order through shared memory: PAPER.md:91), which
