@@ -125,6 +125,7 @@ struct Specialized;           // specialize.cu: model-specialised (NVRTC) kernel
   X(step_mode, -1)             /* bard_step: -1 auto, 0 four launches in sequence, 1 forked, 2 one-launch kernel */ \
   /* read by bard_model_specialize (code generation) */                                                        \
   X(spec_prefetch, 2)          /* bodies of input-load lookahead */                                            \
+  X(spec_prefetch_rnea, 3)     /* ... of the generated RNEA kernel */                                          \
   X(spec_sync, -1)             /* bodies between CTA barriers (0 = none) */                                    \
   X(spec_l2pf, -1)             /* up-front L2 prefetch: 0 never, 1 always, 2 two kernels */                    \
   X(spec_roles, 2)             /* limb roles */                                                                \
