@@ -373,7 +373,9 @@ def test_step_fork_regime_is_measured_at_specialisation():
         m = binding.Model(desc, device=0)
         assert m.get_option("step_fork_regime") == 256 * sms
         m.specialize(ALL + ("fused",))
-        assert m.get_option("step_fork_regime") == want
+        # measured: the humanoid's two-launch step loses by 2x at 4096 (never 3072) and by ~20 % at 16 384 (18 944; 8192 if a noisy box flips it)
+        assert m.get_option("step_fork_regime") in ((want,) if cfg == 0 else (want, 8192))
+        assert m.get_option("step_fork_regime_captured") >= max(8192, m.get_option("step_fork_regime"))
         m.set_option("step_fork_max_b", 1234)
         assert m.get_option("step_fork_regime") == 1234
         m.set_option("step_fork_max_b", -1)
