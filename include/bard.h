@@ -191,7 +191,8 @@ bard_status bard_kinematics(const bard_model* m, int64_t B, const float* q, floa
  * if it is already faster at 4096 (a 7-DOF arm's fused kernel, an 11-DOF spined quadruped -- short walks, and no fork-join on
  * the host: sixteen API calls), from 8192 if it is faster at 16 384, else from 128 x SM count.  Under stream capture the host
  * cost does not exist and forking pays a little longer: bard_step asks the stream (cudaStreamIsCapturing) and then forks up
- * to at least 8192.  Option step_calibrate = 0 replaces the measurement by a static rule on the length of the generated walk
+ * to at least 8192 (so a captured call and a plain call of the same batch may take different forms: their results agree to
+ * rounding, not bit for bit; step_fork_max_b or step_mode pins one form).  Option step_calibrate = 0 replaces the measurement by a static rule on the length of the generated walk
  * (step_light_max).
  * Outputs and layouts as for the four calls. */
 bard_status bard_step(const bard_model* m, int64_t B, const float* q, const float* qd, const float* qdd,
