@@ -1,7 +1,8 @@
 """SURVEY 8(b) "Execution": every operator call only enqueues work on the caller's stream, allocates nothing and never
 synchronises -- so a sequence of calls can be captured into a CUDA graph (bench.py times its trains and the config-2
 rollout that way).  Each entry point is captured once, the graph is replayed on NEW input contents, and the replayed
-results must equal the eager results on the same inputs bit for bit: the forked bard_step (side streams joining the
+results must equal the eager results on the same inputs bit for bit (at batches where the captured and the plain call
+take the same form of bard_step; the last test covers the batches where they do not): the forked bard_step (side streams joining the
 capture), the one-launch and the two-launch bard_step, the single operators of both kernel families, the Euler steps,
 ABA, the RNEA VJP (table-driven, generated, and the static-scratch entry point)."""
 import numpy as np
@@ -123,3 +124,51 @@ def test_dynamics_extras_replay_bit_equal(generated):
             assert torch.equal(a, b)
         assert torch.equal(got[0], got[2]) and torch.equal(got[1], got[3])       # in place == out of place
         assert torch.equal(got[5], got[6])                                       # static scratch == caller workspace
+
+
+@pytest.mark.parametrize("cfg", [0, 2])
+def test_captured_step_may_take_another_form_than_the_plain_call_and_both_match_the_oracle(cfg):
+    """Between the two fork regimes (plain calls: measured, 3072 on these robots; captured calls: at least 8192) a captured
+    bard_step forks the four operators while the plain call is one launch: both are held to the oracle, and they agree to
+    rounding (include/bard.h)."""
+    import oracle
+    dev = torch.device("cuda:0")
+    desc = W.config_robot(cfg)
+    m = binding.Model(desc, device=0)
+    m.specialize(("fk", "jacobian", "rnea", "crba", "fused"))
+    plain, captured = m.get_option("step_fork_regime"), m.get_option("step_fork_regime_captured")
+    assert captured >= max(plain, 8192)
+    B = 5000
+    q, qd, qdd = _state(cfg, B, 0, dev)
+    shapes = ((m.nb, 12, B), (m.nframes, 6, m.nv, B), (m.nv, B), (m.nv, m.nv, B))
+    out = [torch.zeros(s, device=dev) for s in shapes]
+    n0 = binding.launch_count()
+    m.step(B, q, qd, qdd, *out, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    n_plain = binding.launch_count() - n0
+    eager = [o.clone() for o in out]
+    g = _capture(lambda s: m.step(B, q, qd, qdd, *out, s))
+    n0 = binding.launch_count()
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        gg = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(gg, stream=st):
+            m.step(B, q, qd, qdd, *out, torch.cuda.current_stream().cuda_stream)
+    n_captured = binding.launch_count() - n0
+    assert n_plain == (4 if B <= plain else n_plain) and n_captured == (4 if B <= captured else n_captured)
+    for o in out:
+        o.fill_(float("nan"))
+    g.replay()
+    torch.cuda.synchronize()
+    o64 = oracle.Oracle(desc)
+    idx = np.arange(0, B, 25)
+    q64, qd64, qdd64 = (np.ascontiguousarray(t.cpu().numpy()[:, idx].astype(np.float64)) for t in (q, qd, qdd))
+    refs = (o64.fk(q64), o64.jacobian(q64), o64.rnea(q64, qd64, qdd64), o64.crba(q64))
+
+    def nerr(x, ref):
+        return float(np.max(np.abs(np.asarray(x, np.float64) - ref) / np.maximum(1.0, np.abs(ref)))) if ref.size else 0.0
+    for got, e, r, tol in zip(out, eager, refs, (1e-4, 1e-4, 1e-3, 1e-3)):
+        a, b = got.cpu().numpy(), e.cpu().numpy()
+        assert np.isfinite(a).all()
+        assert nerr(a[..., idx], r) <= tol and nerr(b[..., idx], r) <= tol
+        assert nerr(a, b.astype(np.float64)) <= 2 * tol
